@@ -1,0 +1,190 @@
+/*
+ * cdc_seedscan.h -- C ABI of the B200-native brute-force seed scan for a cylindrical drift chamber
+ * (hot path of arXiv 1908.01949, "GPU Tracking in the COMET Phase-I Cylindrical Drift Chamber").
+ *
+ * Citations: PAPER.md:N = line N of the paper text; BJ = BASELINE.json; "reading Cn" = DESIGN.md section 3.
+ *
+ * Conventions
+ *   - plain C, no exceptions cross the boundary.  Every call returns int32_t: CDC_OK or a negative
+ *     cdc_status.  cdc_last_error() gives a thread-local message for the last failing call.
+ *   - units: mm, MeV/c, tesla, radians.
+ *   - pointer names say where the memory lives: h_* = host, d_* = device (cuda:current device).
+ *     All d_* buffers are CALLER-OWNED (the Python binding passes torch tensors' data_ptr()); the
+ *     library never frees them and never keeps them after the call returns (it keeps its own copies
+ *     inside the opaque handles).  Handles are created and destroyed by the library.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls enqueue
+ *     work on it and return without synchronising, except where stated ("synchronises").
+ *   - the seed's linear index, which is also the tie-break order of the argmax, is fixed:
+ *       index = ((((i_theta * n_z + i_z) * n_px + i_px) * n_py + i_py) * n_pz + i_pz
+ *     with axis order (theta0, z0, px0, py0, pz0) (five scanned parameters at R0 = 50 cm).
+ */
+#ifndef CDC_SEEDSCAN_H
+#define CDC_SEEDSCAN_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    CDC_OK = 0,
+    CDC_ERR_INVALID = -1,     /* invalid argument (null pointer, n < 1, h <= 0, duplicate wire id, bad drift ...) */
+    CDC_ERR_RANGE = -2,       /* out of range / table overflow (wire id, field table too small, pool overflow) */
+    CDC_ERR_CUDA = -3,        /* a CUDA runtime call or kernel launch failed */
+    CDC_ERR_NOMEM = -4,       /* host or device allocation failed */
+    CDC_ERR_NOT_READY = -5    /* call order violated (cdc_best_track before cdc_seed_scan) */
+} cdc_status;
+
+typedef struct cdc_geometry cdc_geometry;   /* immutable after create: wire tables + field (A0) */
+typedef struct cdc_events cdc_events;       /* one batch of events: hits, per-wire tables, scan scratch (A1) */
+
+/* Detector description ("eighteen layers with stereo configuration"; numbers from BJ configs[0];
+ * reading C2).  Layer j: waist radius r_mm[j] (radius of the wire at z = 0), n_wires[j] wires at azimuth
+ * phi0_rad[j] + 2 pi k / n_wires[j], signed stereo angle stereo_rad[j].  Wire (j, k) is the line
+ *   w0 = (r cos phi, r sin phi, 0),  u = (-sin(eps) sin phi, sin(eps) cos phi, cos(eps)),  |z| <= z_half_mm.
+ * The fast lookup requires equally spaced layers and equal |stereo| (else CDC_ERR_INVALID).
+ * h_wire: optional canonical per-wire table [W][5] = (w0x, w0y, ux, uy, uz) in fp32 (W = sum n_wires); when
+ * NULL the library builds it from the layer description in fp64 and rounds once to fp32.  Copied. */
+typedef struct {
+    int32_t n_layers;
+    const double *r_mm;
+    const int32_t *n_wires;
+    const double *phi0_rad;
+    const double *stereo_rad;
+    const float *h_wire;
+    double z_half_mm, R0_mm, r_out_mm;      /* 750, 500, 827 */
+} cdc_geometry_desc;
+
+/* Magnetic field ("1T"; PAPER.md:73 the field is uploaded to the GPU; BJ configs[3]; reading C3).
+ * kind 0: uniform (0, 0, bz_T).  kind 1: axisymmetric table, h_br_bz[iz][ir][2] = (B_r, B_z) fp32 at
+ * r = r0_mm + ir dr_mm, z = z0_mm + iz dz_mm, bilinear in (rho, z), cell index clamped to the table.  Copied. */
+typedef struct {
+    int32_t kind;
+    double bz_T;
+    int32_t nr, nz;
+    double r0_mm, z0_mm, dr_mm, dz_mm;
+    const float *h_br_bz;
+} cdc_field_desc;
+
+/* 5-D seed grid of one event: axis a (theta, z, px, py, pz) has n[a] nodes lo[a] + i step[a]. */
+typedef struct {
+    double lo[5], step[5];
+    int32_t n[5];
+} cdc_grid_spec;
+
+/* Propagation and scoring parameters (BJ configs[0]: fixed 2 mm step, <= 1500 steps, 1 mm window).
+ * window_mm: a hit matches iff (D - drift)^2 < lambda = window_mm^2  (Eq. (1), reading C9/C10).
+ * eloss_MeV_per_mm: constant momentum loss per mm of in-gas path (BJ configs[2], reading C6).
+ * rescore_margin: seeds whose fp32 score is within this of the event's fp32 maximum are re-evaluated in
+ * fp64 by cdc_best_track (reading C11); <= 0 selects the default 0.05. */
+typedef struct {
+    double h_mm;
+    int32_t max_steps;
+    double window_mm;
+    double eloss_MeV_per_mm;
+    int32_t charge;                          /* -1 for e-  */
+    double rescore_margin;
+} cdc_scan_params;
+
+/* Hough circle vote (Fig. 4; parametrisation is reading C13): accumulator over circle
+ * centres (cx, cy) in [-half_xy, half_xy) and radii R in [R_lo, R_hi); a hit votes for a bin iff
+ * | |c - x_hit| - R | < tol at the bin centre; bins with | |c| - R | > origin + tol are ineligible. */
+typedef struct {
+    double bin_xy_mm, bin_R_mm, tol_mm, R_lo_mm, R_hi_mm, half_xy_mm, origin_mm;   /* 4, 4, 6, 240, 364, 460, 100 */
+    double half_theta_rad, half_pt_MeV;                                            /* 0.03, 7.5 */
+} cdc_hough_params;
+
+/* Optional per-seed diagnostics of cdc_seed_scan (parity tests): state after the last step. */
+typedef struct {
+    int32_t n_steps, turns, m_gas, pad;
+    double x, y, z;
+} cdc_seed_debug;
+
+/* Counters of the last cdc_seed_scan on an event batch (for throughput / roofline accounting). */
+typedef struct {
+    uint64_t n_seeds;          /* seeds propagated */
+    uint64_t n_steps;          /* RKN steps taken, summed over seeds */
+    uint64_t n_gas_steps;      /* of which started in the gas volume (rho >= R0) */
+    uint64_t n_approach_tests; /* live candidate wires examined (g evaluated) */
+    uint64_t n_pool;           /* candidate-pool entries appended (reading C11) */
+    uint64_t pool_cap;
+} cdc_scan_stats;
+
+const char *cdc_last_error(void);
+
+/* A0: geometry and field tables -> device.  Synchronises.  Errors: INVALID (null, n_layers not in [1, 32],
+ * unequal layer pitch / |stereo|), RANGE (field table does not cover rho <= r_out + 2h_max(=8 mm), |z| <= z_half + 8). */
+int32_t cdc_geometry_create(const cdc_geometry_desc *geom, const cdc_field_desc *field, cdc_geometry **out);
+int32_t cdc_geometry_destroy(cdc_geometry *g);
+/* Copy the canonical fp32 wire table [W][5] to host memory (W returned through n_wires_total if non-null). */
+int32_t cdc_geometry_wire_table(const cdc_geometry *g, float *h_wire_or_null, int32_t *n_wires_total);
+
+/* A1: hits of a batch of events -> library-owned device copies, a dense per-wire drift table
+ * (sentinel -1 = no hit) and a per-wire hit bitmask per event (hits uploaded to the GPU;
+ * BJ north_star: "hits binned by (layer, phi-cell) so each step's lookup is O(1)").
+ * h_hit_offsets: host, n_events + 1 prefix offsets into wire_id / drift_mm.  wire_id / drift_mm live on the
+ * host (hits_on_device = 0) or on the device (1).  Hits need not be sorted.  Synchronises (validation result).
+ * Errors: RANGE wire id outside [0, W); INVALID duplicate wire id within an event, drift < 0 or non-finite. */
+int32_t cdc_event_upload(const cdc_geometry *g, int32_t n_events, const int32_t *h_hit_offsets,
+                         const int32_t *wire_id, const float *drift_mm, int32_t hits_on_device,
+                         void *stream, cdc_events **out);
+int32_t cdc_events_destroy(cdc_events *ev);
+/* Copy the A1 tables to host memory: h_drift_of_wire [n_events][W] f32, h_hit_bits [n_events][ceil(W/32)] u32
+ * (either may be NULL).  Synchronises. */
+int32_t cdc_events_tables(const cdc_events *ev, float *h_drift_of_wire, uint32_t *h_hit_bits);
+
+/* A2: Hough pre-vote.  d_zref_mm[e]: z at which the stereo wires' (x, y) are taken.
+ * Outputs per event: d_ranges[e][3][2] = (lo, hi) of theta0, px0, py0 (f64); d_peak[e][4] = (iR, icy, icx, votes)
+ * with ties to the lowest linear bin index; d_accum_or_null[e][nR][ncy][ncx] u32 (full accumulator, optional).
+ * The field's bz_T and params->charge fix the sense of rotation. */
+int32_t cdc_hough_dims(const cdc_hough_params *hp, int32_t *dims3 /* nR, ncy, ncx */);
+int32_t cdc_hough_seed_ranges(const cdc_geometry *g, const cdc_events *ev, const cdc_hough_params *hp,
+                              int32_t charge, const float *d_zref_mm, double *d_ranges, int32_t *d_peak,
+                              uint32_t *d_accum_or_null, void *stream);
+
+/* A3-A7: the seed scan.  Every seed of every event's grid is propagated by Nystroem-RK4 (PAPER.md:55,
+ * reading C5) in fp32 with compensated state, wires near each step are looked up (reading C8), owned
+ * approaches to fired wires are scored (readings C9/C10), and the per-event maximum of
+ * S = n_match - chi2 / lambda is reduced into d_best_key[e] = (bits(S_fp32) << 32) | (0xFFFFFFFF - index).
+ * h_grids: host, one spec per event (product of n <= 2^31 - 1, each n <= 4096).
+ * d_n_match_or_null / d_chi2_or_null: per-seed outputs, events concatenated in grid order (sum of n_seeds).
+ * d_debug_or_null: cdc_seed_debug per seed.  Seeds close to the running maximum are appended to the
+ * library-owned candidate pool of `ev` for cdc_best_track.  Asynchronous. */
+int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec *h_grids,
+                      const cdc_scan_params *params, uint32_t *d_n_match_or_null, float *d_chi2_or_null,
+                      cdc_seed_debug *d_debug_or_null, uint64_t *d_best_key, void *stream);
+/* Counters of the last scan.  Synchronises `stream`. */
+int32_t cdc_scan_get_stats(const cdc_events *ev, cdc_scan_stats *h_out, void *stream);
+
+/* A8-A9: exact best seed and hit -> turn labels ("lowest E", "hits with d^2 < lambda are
+ * classified"; readings C11/C12).  Pool candidates within rescore_margin of the fp32 maximum are re-evaluated
+ * in IEEE fp64 without FMA contraction; the maximum of S (ties: lowest index) is the best seed; its matched
+ * approaches label each hit with a turn index, or -1.  Per event: d_best_seed i64, d_best_n_match u32,
+ * d_best_chi2 f64; d_labels i32 per hit (events concatenated in upload order).  Must follow cdc_seed_scan on
+ * the same stream with the same grids / params.  Asynchronous; pool overflow is reported by the next
+ * cdc_scan_get_stats (n_pool > pool_cap) and by cdc_find_tracks_host. */
+int32_t cdc_best_track(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec *h_grids,
+                       const cdc_scan_params *params, const uint64_t *d_best_key, int64_t *d_best_seed,
+                       uint32_t *d_best_n_match, double *d_best_chi2, int32_t *d_labels, void *stream);
+
+/* The whole path with host buffers in and out (upload, optional Hough ranges, scan, best track, read-back):
+ * the end-to-end call.  If hp is non-NULL the (theta, px, py) axes of every grid are replaced by n[a] nodes
+ * spanning the Hough ranges (BJ configs[2]); h_zref_mm is then required.  Outputs (host): h_best_seed,
+ * h_best_n_match, h_best_chi2, h_best_key per event; h_labels per hit; h_ranges_or_null [n_events][3][2].
+ * Synchronises. */
+int32_t cdc_find_tracks_host(const cdc_geometry *g, int32_t n_events, const int32_t *h_hit_offsets,
+                             const int32_t *h_wire_id, const float *h_drift_mm, const cdc_grid_spec *h_grids,
+                             const cdc_scan_params *params, const cdc_hough_params *hp_or_null,
+                             const float *h_zref_mm_or_null, int64_t *h_best_seed, uint32_t *h_best_n_match,
+                             double *h_best_chi2, uint64_t *h_best_key, int32_t *h_labels,
+                             double *h_ranges_or_null, void *stream);
+
+/* Register-only FFMA chain: the empirical FP32 peak used as the roofline denominator.  Runs `iters`
+ * dependent-chain iterations on every SM, returns achieved FLOP/s (2 per FFMA).  Synchronises. */
+int32_t cdc_fp32_peak_probe(int32_t iters, double *h_flops_per_s, double *h_ms, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CDC_SEEDSCAN_H */

@@ -1,0 +1,98 @@
+// C ABI, part 2: A1 event upload / binning and the events handle.
+#include <math.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+
+#include "cdc_internal.cuh"
+
+namespace {
+
+void free_events(cdc_events *ev)
+{
+    if (!ev) return;
+    cudaFree(ev->d_offsets); cudaFree(ev->d_wire_id); cudaFree(ev->d_drift); cudaFree(ev->d_drift_tab);
+    cudaFree(ev->d_bits); cudaFree(ev->d_err); cudaFree(ev->axes.d); cudaFree(ev->d_grids); cudaFree(ev->d_pool);
+    cudaFree(ev->d_counters); cudaFree(ev->d_pool_S64); cudaFree(ev->d_pool_chi2); cudaFree(ev->d_pool_nmatch);
+    cudaFree(ev->d_ev_maxS); cudaFree(ev->d_ev_best); cudaFree(ev->d_wire_label); cudaFree(ev->d_wire_best);
+    cudaFree(ev->d_peak_key);
+    delete ev;
+}
+
+}  // namespace
+
+#define EV_CUDA(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { free_events(ev); \
+    cdc_set_error(std::string(#expr) + ": " + cudaGetErrorString(e_)); \
+    return e_ == cudaErrorMemoryAllocation ? CDC_ERR_NOMEM : CDC_ERR_CUDA; } } while (0)
+
+extern "C" int32_t cdc_event_upload(const cdc_geometry *g, int32_t n_events, const int32_t *h_hit_offsets,
+                                    const int32_t *wire_id, const float *drift_mm, int32_t hits_on_device,
+                                    void *stream, cdc_events **out)
+{
+    if (!g || !h_hit_offsets || !out) CDC_FAIL(CDC_ERR_INVALID, "cdc_event_upload: null argument");
+    *out = nullptr;
+    if (n_events < 1 || n_events > 65535) CDC_FAIL(CDC_ERR_INVALID, "cdc_event_upload: n_events must be in [1, 65535]");
+    if (h_hit_offsets[0] != 0) CDC_FAIL(CDC_ERR_INVALID, "cdc_event_upload: hit_offsets[0] must be 0");
+    int32_t max_hits = 0;
+    for (int e = 0; e < n_events; ++e) {
+        const int32_t c = h_hit_offsets[e + 1] - h_hit_offsets[e];
+        if (c < 0) CDC_FAIL(CDC_ERR_INVALID, "cdc_event_upload: hit_offsets must be non-decreasing");
+        max_hits = std::max(max_hits, c);
+    }
+    const int32_t total = h_hit_offsets[n_events];
+    if (total > 0 && (!wire_id || !drift_mm)) CDC_FAIL(CDC_ERR_INVALID, "cdc_event_upload: null hit arrays");
+    cudaStream_t s = (cudaStream_t)stream;
+    cdc_events *ev = new (std::nothrow) cdc_events;
+    if (!ev) CDC_FAIL(CDC_ERR_NOMEM, "cdc_event_upload: host allocation failed");
+    ev->geom = g; ev->n_events = n_events; ev->total_hits = total; ev->W = g->W; ev->n_bit_words = (g->W + 31) / 32;
+    ev->max_hits_per_event = max_hits;
+    ev->offsets.assign(h_hit_offsets, h_hit_offsets + n_events + 1);
+    const size_t nt = std::max<size_t>((size_t)total, 1);
+    EV_CUDA(cudaMalloc((void **)&ev->d_offsets, sizeof(int32_t) * (size_t)(n_events + 1)));
+    EV_CUDA(cudaMalloc((void **)&ev->d_wire_id, sizeof(int32_t) * nt));
+    EV_CUDA(cudaMalloc((void **)&ev->d_drift, sizeof(float) * nt));
+    EV_CUDA(cudaMalloc((void **)&ev->d_drift_tab, sizeof(float) * (size_t)n_events * g->W));
+    EV_CUDA(cudaMalloc((void **)&ev->d_bits, sizeof(uint32_t) * (size_t)n_events * ev->n_bit_words));
+    EV_CUDA(cudaMalloc((void **)&ev->d_err, sizeof(int32_t)));
+    EV_CUDA(cudaMalloc((void **)&ev->d_counters, sizeof(unsigned long long) * CNT_N));
+    EV_CUDA(cudaMalloc((void **)&ev->d_ev_maxS, sizeof(unsigned long long) * (size_t)n_events));
+    EV_CUDA(cudaMalloc((void **)&ev->d_ev_best, sizeof(unsigned long long) * (size_t)n_events));
+    EV_CUDA(cudaMalloc((void **)&ev->d_peak_key, sizeof(unsigned long long) * (size_t)n_events));
+    EV_CUDA(cudaMalloc((void **)&ev->d_wire_label, sizeof(int32_t) * (size_t)n_events * g->W));
+    EV_CUDA(cudaMalloc((void **)&ev->d_wire_best, sizeof(double) * (size_t)n_events * g->W));
+    EV_CUDA(cudaMalloc((void **)&ev->d_grids, sizeof(GridDev) * (size_t)n_events));
+    EV_CUDA(cudaMemsetAsync(ev->d_counters, 0, sizeof(unsigned long long) * CNT_N, s));
+    EV_CUDA(cudaMemcpyAsync(ev->d_offsets, h_hit_offsets, sizeof(int32_t) * (size_t)(n_events + 1), cudaMemcpyHostToDevice, s));
+    if (total > 0) {
+        const cudaMemcpyKind k = hits_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+        EV_CUDA(cudaMemcpyAsync(ev->d_wire_id, wire_id, sizeof(int32_t) * (size_t)total, k, s));
+        EV_CUDA(cudaMemcpyAsync(ev->d_drift, drift_mm, sizeof(float) * (size_t)total, k, s));
+    }
+    EV_CUDA(launch_bin_events(n_events, g->W, ev->n_bit_words, max_hits, ev->d_offsets, ev->d_wire_id, ev->d_drift,
+                              ev->d_drift_tab, ev->d_bits, ev->d_err, s));
+    int32_t err = 0;
+    EV_CUDA(cudaMemcpyAsync(&err, ev->d_err, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    EV_CUDA(cudaStreamSynchronize(s));
+    if (err & 1) { free_events(ev); CDC_FAIL(CDC_ERR_RANGE, "cdc_event_upload: wire id out of range"); }
+    if (err & 2) { free_events(ev); CDC_FAIL(CDC_ERR_INVALID, "cdc_event_upload: drift distance negative or non-finite"); }
+    if (err & 4) { free_events(ev); CDC_FAIL(CDC_ERR_INVALID, "cdc_event_upload: duplicate wire id within an event"); }
+    *out = ev;
+    return CDC_OK;
+}
+
+extern "C" int32_t cdc_events_destroy(cdc_events *ev)
+{
+    free_events(ev);
+    return CDC_OK;
+}
+
+extern "C" int32_t cdc_events_tables(const cdc_events *ev, float *h_drift_of_wire, uint32_t *h_hit_bits)
+{
+    if (!ev) CDC_FAIL(CDC_ERR_INVALID, "cdc_events_tables: null events");
+    if (h_drift_of_wire)
+        CDC_CUDA(cudaMemcpy(h_drift_of_wire, ev->d_drift_tab, sizeof(float) * (size_t)ev->n_events * ev->W, cudaMemcpyDeviceToHost));
+    if (h_hit_bits)
+        CDC_CUDA(cudaMemcpy(h_hit_bits, ev->d_bits, sizeof(uint32_t) * (size_t)ev->n_events * ev->n_bit_words, cudaMemcpyDeviceToHost));
+    return CDC_OK;
+}

@@ -1,0 +1,199 @@
+// C ABI, part 3: A2 Hough ranges, A3-A7 seed scan, A8-A9 best track.
+#include <math.h>
+#include <string.h>
+
+#include <algorithm>
+
+#include "cdc_internal.cuh"
+
+namespace {
+
+constexpr uint32_t kPoolCap = 1u << 20;
+constexpr double kDefaultMargin = 0.05;
+
+int32_t check_params(const cdc_scan_params *p, const char *who)
+{
+    if (!p) CDC_FAIL(CDC_ERR_INVALID, std::string(who) + ": null params");
+    if (!(p->h_mm > 0.0) || !(p->h_mm <= 4.0)) CDC_FAIL(CDC_ERR_INVALID, std::string(who) + ": need 0 < h <= 4 mm");
+    if (p->max_steps < 1) CDC_FAIL(CDC_ERR_INVALID, std::string(who) + ": max_steps < 1");
+    if (!(p->window_mm > 0.0)) CDC_FAIL(CDC_ERR_INVALID, std::string(who) + ": window <= 0");
+    if (!(p->eloss_MeV_per_mm >= 0.0)) CDC_FAIL(CDC_ERR_INVALID, std::string(who) + ": negative energy loss");
+    if (p->charge != 1 && p->charge != -1) CDC_FAIL(CDC_ERR_INVALID, std::string(who) + ": charge must be +-1");
+    return CDC_OK;
+}
+
+// A3 host part: validate the grids, build the fp64 axis tables and the per-event grid records
+int32_t prepare_grids(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec *grids, cudaStream_t s)
+{
+    const int E = ev->n_events;
+    int32_t stride = 1;
+    ev->h_grids.resize(E);
+    int64_t off = 0;
+    for (int e = 0; e < E; ++e) {
+        int64_t prod = 1;
+        for (int a = 0; a < 5; ++a) {
+            const int32_t n = grids[e].n[a];
+            if (n < 1 || n > CDC_MAX_AXIS) CDC_FAIL(CDC_ERR_INVALID, "cdc_seed_scan: grid n must be in [1, 4096]");
+            if (!isfinite(grids[e].lo[a]) || !isfinite(grids[e].step[a]))
+                CDC_FAIL(CDC_ERR_INVALID, "cdc_seed_scan: non-finite grid lo / step");
+            prod *= n;
+            if (prod > 2147483647LL) CDC_FAIL(CDC_ERR_INVALID, "cdc_seed_scan: more than 2^31 - 1 seeds in a grid");
+            stride = std::max(stride, n);
+            ev->h_grids[e].n[a] = n;
+        }
+        ev->h_grids[e].n_seeds = (int32_t)prod;
+        ev->h_grids[e].out_offset = off;
+        off += prod;
+    }
+    if (ev->axes.stride < stride) {
+        cudaFree(ev->axes.d); ev->axes.d = nullptr; ev->axes.stride = 0;
+        CDC_CUDA(cudaMalloc((void **)&ev->axes.d, sizeof(double) * (size_t)E * 6 * stride));
+        ev->axes.stride = stride;
+    }
+    stride = ev->axes.stride;
+    std::vector<double> tab((size_t)E * 6 * stride, 0.0);
+    for (int e = 0; e < E; ++e) {
+        double *t = tab.data() + (size_t)e * 6 * stride;
+        const cdc_grid_spec &G = grids[e];
+        for (int i = 0; i < G.n[0]; ++i) {            // reading C4: r0 = (R0 cos(theta), R0 sin(theta), z)
+            const double th = G.lo[0] + (double)i * G.step[0];
+            t[i] = g->R0 * cos(th);
+            t[stride + i] = g->R0 * sin(th);
+        }
+        for (int a = 1; a < 5; ++a)
+            for (int i = 0; i < G.n[a]; ++i) t[(size_t)(a + 1) * stride + i] = G.lo[a] + (double)i * G.step[a];
+    }
+    CDC_CUDA(cudaMemcpyAsync(ev->axes.d, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice, s));
+    CDC_CUDA(cudaMemcpyAsync(ev->d_grids, ev->h_grids.data(), sizeof(GridDev) * (size_t)E, cudaMemcpyHostToDevice, s));
+    CDC_CUDA(cudaStreamSynchronize(s));               // `tab` is pageable and about to go out of scope
+    return CDC_OK;
+}
+
+int32_t ensure_pool(cdc_events *ev)
+{
+    if (ev->d_pool) return CDC_OK;
+    const uint32_t cap = std::max<uint32_t>(kPoolCap, 256u * (uint32_t)ev->n_events);
+    CDC_CUDA(cudaMalloc((void **)&ev->d_pool, sizeof(PoolEntry) * (size_t)cap));
+    CDC_CUDA(cudaMalloc((void **)&ev->d_pool_S64, sizeof(double) * (size_t)cap));
+    CDC_CUDA(cudaMalloc((void **)&ev->d_pool_chi2, sizeof(double) * (size_t)cap));
+    CDC_CUDA(cudaMalloc((void **)&ev->d_pool_nmatch, sizeof(int32_t) * (size_t)cap));
+    ev->pool_cap = cap;
+    return CDC_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------ A2
+extern "C" int32_t cdc_hough_dims(const cdc_hough_params *hp, int32_t *dims3)
+{
+    if (!hp || !dims3) CDC_FAIL(CDC_ERR_INVALID, "cdc_hough_dims: null argument");
+    if (!(hp->bin_xy_mm > 0) || !(hp->bin_R_mm > 0) || !(hp->R_hi_mm > hp->R_lo_mm) || !(hp->half_xy_mm > 0) || !(hp->tol_mm > 0))
+        CDC_FAIL(CDC_ERR_INVALID, "cdc_hough_dims: bad Hough parameters");
+    dims3[0] = (int32_t)floor((hp->R_hi_mm - hp->R_lo_mm) / hp->bin_R_mm + 0.5);
+    dims3[1] = (int32_t)floor(2.0 * hp->half_xy_mm / hp->bin_xy_mm + 0.5);
+    dims3[2] = dims3[1];
+    if (dims3[0] < 1 || dims3[1] < 1 || (int64_t)dims3[0] * dims3[1] * dims3[2] > 0x7FFFFFFFLL || dims3[0] > 256)
+        CDC_FAIL(CDC_ERR_RANGE, "cdc_hough_dims: accumulator too large (nR <= 256, bins < 2^31)");
+    return CDC_OK;
+}
+
+extern "C" int32_t cdc_hough_seed_ranges(const cdc_geometry *g, const cdc_events *ev, const cdc_hough_params *hp,
+                                         int32_t charge, const float *d_zref_mm, double *d_ranges, int32_t *d_peak,
+                                         uint32_t *d_accum_or_null, void *stream)
+{
+    if (!g || !ev || !hp || !d_zref_mm || !d_ranges || !d_peak) CDC_FAIL(CDC_ERR_INVALID, "cdc_hough_seed_ranges: null argument");
+    if (ev->geom != g) CDC_FAIL(CDC_ERR_INVALID, "cdc_hough_seed_ranges: events belong to another geometry");
+    if (charge != 1 && charge != -1) CDC_FAIL(CDC_ERR_INVALID, "cdc_hough_seed_ranges: charge must be +-1");
+    int32_t dims[3];
+    const int32_t rc = cdc_hough_dims(hp, dims);
+    if (rc != CDC_OK) return rc;
+    HoughLaunch L;
+    L.n_events = ev->n_events; L.nR = dims[0]; L.ncy = dims[1]; L.ncx = dims[2];
+    L.bin_xy = (float)hp->bin_xy_mm; L.bin_R = (float)hp->bin_R_mm; L.tol = (float)hp->tol_mm; L.R_lo = (float)hp->R_lo_mm;
+    L.half_xy = (float)hp->half_xy_mm; L.origin = (float)hp->origin_mm;
+    L.bin_xy64 = hp->bin_xy_mm; L.bin_R64 = hp->bin_R_mm; L.R_lo64 = hp->R_lo_mm; L.half_xy64 = hp->half_xy_mm;
+    L.R0 = g->R0; L.half_theta = hp->half_theta_rad; L.half_pt = hp->half_pt_MeV; L.bz = g->field.bz_T; L.charge = charge;
+    L.d_wire5 = g->d_wire5; L.d_offsets = ev->d_offsets; L.d_wire_id = ev->d_wire_id; L.d_zref = d_zref_mm;
+    L.d_ranges = d_ranges; L.d_peak = d_peak; L.d_accum = d_accum_or_null; L.d_peak_key = ev->d_peak_key;
+    CDC_CUDA(launch_hough(L, (cudaStream_t)stream));
+    return CDC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ A3-A7
+extern "C" int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec *h_grids,
+                                 const cdc_scan_params *p, uint32_t *d_n_match, float *d_chi2,
+                                 cdc_seed_debug *d_debug, uint64_t *d_best_key, void *stream)
+{
+    if (!g || !ev || !h_grids || !d_best_key) CDC_FAIL(CDC_ERR_INVALID, "cdc_seed_scan: null argument");
+    if (ev->geom != g) CDC_FAIL(CDC_ERR_INVALID, "cdc_seed_scan: events belong to another geometry");
+    int32_t rc = check_params(p, "cdc_seed_scan");
+    if (rc != CDC_OK) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    if ((rc = prepare_grids(g, ev, h_grids, s)) != CDC_OK) return rc;
+    if ((rc = ensure_pool(ev)) != CDC_OK) return rc;
+    CDC_CUDA(cudaMemsetAsync(d_best_key, 0, sizeof(uint64_t) * (size_t)ev->n_events, s));
+    CDC_CUDA(cudaMemsetAsync(ev->d_counters, 0, sizeof(unsigned long long) * CNT_N, s));
+    ScanLaunch L;
+    L.gd = g->gd; L.fd = g->fd; L.n_events = ev->n_events; L.d_grids = ev->d_grids; L.d_axes = ev->axes.d;
+    L.axis_stride = ev->axes.stride; L.d_drift_tab = ev->d_drift_tab; L.d_bits = ev->d_bits;
+    L.h = (float)p->h_mm; L.h64 = p->h_mm; L.lambda = (float)(p->window_mm * p->window_mm);
+    L.eloss_h = (float)(p->eloss_MeV_per_mm * p->h_mm);
+    L.max_steps = p->max_steps; L.charge = p->charge;
+    L.margin = (float)(p->rescore_margin > 0.0 ? p->rescore_margin : kDefaultMargin);
+    L.d_n_match = d_n_match; L.d_chi2 = d_chi2; L.d_debug = d_debug; L.d_best_key = d_best_key;
+    L.d_pool = ev->d_pool; L.pool_cap = ev->pool_cap; L.d_counters = ev->d_counters;
+    L.max_seeds_per_event = 0;
+    for (const GridDev &G : ev->h_grids) L.max_seeds_per_event = std::max<int64_t>(L.max_seeds_per_event, G.n_seeds);
+    CDC_CUDA(launch_seed_scan(L, s));
+    ev->scanned = true;
+    return CDC_OK;
+}
+
+extern "C" int32_t cdc_scan_get_stats(const cdc_events *ev, cdc_scan_stats *out, void *stream)
+{
+    if (!ev || !out) CDC_FAIL(CDC_ERR_INVALID, "cdc_scan_get_stats: null argument");
+    if (!ev->scanned) CDC_FAIL(CDC_ERR_NOT_READY, "cdc_scan_get_stats: no scan has run on these events");
+    unsigned long long c[CNT_N];
+    CDC_CUDA(cudaMemcpyAsync(c, ev->d_counters, sizeof(c), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CDC_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    out->n_seeds = 0;
+    for (const GridDev &G : ev->h_grids) out->n_seeds += (uint64_t)G.n_seeds;
+    out->n_steps = c[CNT_STEPS]; out->n_gas_steps = c[CNT_GAS]; out->n_approach_tests = c[CNT_TESTS];
+    out->n_pool = c[CNT_POOL]; out->pool_cap = ev->pool_cap;
+    return CDC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ A8-A9
+extern "C" int32_t cdc_best_track(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec *h_grids,
+                                  const cdc_scan_params *p, const uint64_t *d_best_key, int64_t *d_best_seed,
+                                  uint32_t *d_best_n_match, double *d_best_chi2, int32_t *d_labels, void *stream)
+{
+    if (!g || !ev || !h_grids || !d_best_key || !d_best_seed || !d_best_n_match || !d_best_chi2)
+        CDC_FAIL(CDC_ERR_INVALID, "cdc_best_track: null argument");
+    if (ev->geom != g) CDC_FAIL(CDC_ERR_INVALID, "cdc_best_track: events belong to another geometry");
+    if (!ev->scanned) CDC_FAIL(CDC_ERR_NOT_READY, "cdc_best_track: call cdc_seed_scan first");
+    int32_t rc = check_params(p, "cdc_best_track");
+    if (rc != CDC_OK) return rc;
+    for (int e = 0; e < ev->n_events; ++e)
+        for (int a = 0; a < 5; ++a)
+            if (h_grids[e].n[a] != ev->h_grids[e].n[a]) CDC_FAIL(CDC_ERR_INVALID, "cdc_best_track: grids differ from the scanned ones");
+    BestLaunch L;
+    L.g = g->g64; L.n_events = ev->n_events; L.d_grids = ev->d_grids; L.d_axes = ev->axes.d; L.axis_stride = ev->axes.stride;
+    L.d_offsets = ev->d_offsets; L.d_wire_id = ev->d_wire_id; L.d_drift = ev->d_drift; L.d_drift_tab = ev->d_drift_tab;
+    L.d_bits = ev->d_bits; L.W = ev->W; L.n_bit_words = ev->n_bit_words; L.max_hits_per_event = ev->max_hits_per_event;
+    L.h = p->h_mm; L.window = p->window_mm; L.eloss = p->eloss_MeV_per_mm; L.max_steps = p->max_steps; L.charge = p->charge;
+    L.margin = (float)(p->rescore_margin > 0.0 ? p->rescore_margin : kDefaultMargin);
+    L.d_best_key = d_best_key; L.d_pool = ev->d_pool; L.pool_cap = ev->pool_cap; L.d_counters = ev->d_counters;
+    L.d_pool_S64 = ev->d_pool_S64; L.d_pool_chi2 = ev->d_pool_chi2; L.d_pool_nmatch = ev->d_pool_nmatch;
+    L.d_ev_maxS = ev->d_ev_maxS; L.d_ev_best = ev->d_ev_best; L.d_wire_label = ev->d_wire_label; L.d_wire_best = ev->d_wire_best;
+    L.d_best_seed = d_best_seed; L.d_best_n_match = d_best_n_match; L.d_best_chi2 = d_best_chi2; L.d_labels = d_labels;
+    CDC_CUDA(launch_best_track(L, (cudaStream_t)stream));
+    return CDC_OK;
+}
+
+extern "C" int32_t cdc_fp32_peak_probe(int32_t iters, double *h_flops_per_s, double *h_ms, void *stream)
+{
+    if (iters < 1) CDC_FAIL(CDC_ERR_INVALID, "cdc_fp32_peak_probe: iters < 1");
+    CDC_CUDA(run_fp32_peak_probe(iters, h_flops_per_s, h_ms, (cudaStream_t)stream));
+    return CDC_OK;
+}

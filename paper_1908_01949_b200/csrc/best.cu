@@ -1,0 +1,299 @@
+// A8-A9: exact re-score of the near-best seeds and hit -> turn labels of the best seed.
+//
+// THIS FILE IS COMPILED WITH -fmad=false: every fp64 +, -, *, /, sqrt below is a single IEEE-754 operation in
+// the order DESIGN.md section 3 (readings C4-C10, C12) writes the formulas, left to right, so the result is a
+// function of the inputs only and can be compared bit for bit with any other IEEE evaluation of the same
+// formulas (reading C11).  Transcendentals appear only where they cannot change the result: in the choice of
+// candidate wires (a superset by construction, reading C8).
+//
+//   PAPER.md:55      RKN propagation                           -> rkn_step64()
+//   PAPER.md:55,:69  DCA, left/right ambiguity                 -> eval_seed64()
+//   PAPER.md:65-69   Eq. (1), S = n_match - chi2 / lambda      -> rescore_kernel / pick_kernel
+//   PAPER.md:69      "hits with d^2 < lambda are classified"   -> label_kernel
+#include "cdc_internal.cuh"
+
+namespace {
+
+struct BestArgs {
+    Geom64 g;
+    const GridDev *grids;
+    const double *axes;
+    int32_t axis_stride;
+    const float *drift_tab;
+    const uint32_t *bits;
+    int32_t W, n_bit_words;
+    double h, lambda, eloss_h, kq;
+    int32_t max_steps;
+};
+
+__device__ __forceinline__ void field64(const Geom64 &g, double x, double y, double z, double *B)
+{
+    if (g.field_kind == 0) { B[0] = 0.0; B[1] = 0.0; B[2] = g.bz; return; }
+    const double rho = sqrt(x * x + y * y);
+    const double fr = (rho - g.r0) / g.dr;
+    const double fz = (z - g.z0) / g.dz;
+    int ir = (int)floor(fr), iz = (int)floor(fz);
+    ir = max(0, min(ir, g.nr - 2));
+    iz = max(0, min(iz, g.nz - 2));
+    const double wr = fr - (double)ir, wz = fz - (double)iz;
+    const float *n00 = g.tab + ((size_t)iz * g.nr + ir) * 2;
+    const float *n01 = n00 + 2, *n10 = n00 + (size_t)g.nr * 2, *n11 = n10 + 2;
+    const double Br = (1.0 - wz) * ((1.0 - wr) * (double)n00[0] + wr * (double)n01[0])
+                    + wz * ((1.0 - wr) * (double)n10[0] + wr * (double)n11[0]);
+    const double Bz = (1.0 - wz) * ((1.0 - wr) * (double)n00[1] + wr * (double)n01[1])
+                    + wz * ((1.0 - wr) * (double)n10[1] + wr * (double)n11[1]);
+    if (rho > 0.0) { B[0] = Br * x / rho; B[1] = Br * y / rho; }
+    else { B[0] = 0.0; B[1] = 0.0; }
+    B[2] = Bz;
+}
+
+__device__ __forceinline__ void lorentz64(double a, const double *T, const double *B, double *k)
+{
+    k[0] = a * (T[1] * B[2] - T[2] * B[1]);
+    k[1] = a * (T[2] * B[0] - T[0] * B[2]);
+    k[2] = a * (T[0] * B[1] - T[1] * B[0]);
+}
+
+// reading C5: the four stages and the update, each expression evaluated left to right
+__device__ void rkn_step64(const Geom64 &g, double a, double h, const double *r, const double *T, double *rn,
+                           double *Tn)
+{
+    double B[3], k1[3], k2[3], k3[3], k4[3], q[3], U[3];
+    const double hh = h / 2.0, h28 = h * h / 8.0, h22 = h * h / 2.0, h26 = h * h / 6.0, h6 = h / 6.0;
+    field64(g, r[0], r[1], r[2], B);
+    lorentz64(a, T, B, k1);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { q[i] = r[i] + hh * T[i] + h28 * k1[i]; U[i] = T[i] + hh * k1[i]; }
+    field64(g, q[0], q[1], q[2], B);
+    lorentz64(a, U, B, k2);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) U[i] = T[i] + hh * k2[i];
+    lorentz64(a, U, B, k3);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { q[i] = r[i] + h * T[i] + h22 * k3[i]; U[i] = T[i] + h * k3[i]; }
+    field64(g, q[0], q[1], q[2], B);
+    lorentz64(a, U, B, k4);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        rn[i] = r[i] + h * T[i] + h26 * (k1[i] + k2[i] + k3[i]);
+        Tn[i] = T[i] + h6 * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
+    }
+}
+
+// reading C9: delta = d - (d.u) u with d = r - w0;  returns g = delta . T when T != nullptr
+__device__ __forceinline__ void wire_offset64(const float *w, const double *r, double *delta, double *tpar)
+{
+    const double dx = r[0] - (double)w[0], dy = r[1] - (double)w[1], dz = r[2];
+    const double ux = (double)w[2], uy = (double)w[3], uz = (double)w[4];
+    const double t = dx * ux + dy * uy + dz * uz;
+    delta[0] = dx - t * ux; delta[1] = dy - t * uy; delta[2] = dz - t * uz;
+    *tpar = t;
+}
+
+// candidate wires around r: 3 nearest layers x 3 nearest cells, those with a hit, ascending wire id
+// (fp32 is enough: the set only has to contain every wire within ~9.3 mm, reading C8)
+__device__ int candidates64(const Geom64 &g, const uint32_t *bits, const double *r, int *cand)
+{
+    const float x = (float)r[0], y = (float)r[1], z = (float)r[2];
+    const float zeta = z * g.tan_abs;
+    const float u2 = x * x + y * y - zeta * zeta;
+    if (!(u2 > 0.0f)) return 0;
+    const float fj = (sqrtf(u2) - g.r_first) * g.inv_pitch;
+    if (fj < -1.0f || fj > (float)g.n_layers) return 0;
+    const int jc = (int)rintf(fj);
+    const float phi = atan2f(y, x);
+    int n = 0;
+    for (int j = jc - 1; j <= jc + 1; ++j) {
+        if (j < 0 || j >= g.n_layers) continue;
+        const LayerDev L = g.layers[j];
+        const float kf = (phi - L.phi0 - atanf(z * L.shift_k)) * L.kscale;
+        const int kc = (int)rintf(kf);
+        for (int dk = -1; dk <= 1; ++dk) {
+            int k = (kc + dk) % L.n;
+            if (k < 0) k += L.n;
+            const int w = L.offset + k;
+            if (!((bits[w >> 5] >> (w & 31)) & 1u)) continue;
+            int i = n++;
+            while (i > 0 && cand[i - 1] > w) { cand[i] = cand[i - 1]; --i; }   // insertion sort, ascending id
+            cand[i] = w;
+        }
+    }
+    return n;
+}
+
+struct Eval64 {
+    int32_t n_match, n_steps, turns, m_gas;
+    double chi2;
+};
+
+// readings C4-C10: evaluate one seed.  wire_label / wire_best (optional, per wire of this event): reading C12.
+__device__ void eval_seed64(const BestArgs &A, int e, uint32_t index, Eval64 &out, int32_t *wire_label,
+                            double *wire_best)
+{
+    const GridDev G = A.grids[e];
+    uint32_t q = index;
+    const int i_pz = q % G.n[4]; q /= G.n[4];
+    const int i_py = q % G.n[3]; q /= G.n[3];
+    const int i_px = q % G.n[2]; q /= G.n[2];
+    const int i_z = q % G.n[1];
+    const int i_th = q / G.n[1];
+    const double *ax = A.axes + (size_t)e * 6 * A.axis_stride;
+    const double px = ax[3 * A.axis_stride + i_px], py = ax[4 * A.axis_stride + i_py], pz = ax[5 * A.axis_stride + i_pz];
+    double r[3] = {ax[i_th], ax[A.axis_stride + i_th], ax[2 * A.axis_stride + i_z]};     // C4
+    const double p0 = sqrt(px * px + py * py + pz * pz);
+    double T[3] = {px / p0, py / p0, pz / p0};
+    double p = p0, chi2 = 0.0;
+    const uint32_t *bits = A.bits + (size_t)e * A.n_bit_words;
+    const float *drift = A.drift_tab + (size_t)e * A.W;
+    int n = 0, turn = 0, m = 0, n_match = 0;
+    bool cn = true;
+    int cand[9];
+    while (n < A.max_steps) {
+        const double a = A.kq / p;
+        double rn[3], Tn[3];
+        rkn_step64(A.g, a, A.h, r, T, rn, Tn);
+        if (cn) {
+            const int nc = candidates64(A.g, bits, r, cand);
+            for (int ic = 0; ic < nc; ++ic) {
+                const int w = cand[ic];
+                const float *wr = A.g.wire5 + (size_t)w * 5;
+                double d0[3], d1[3], tp;
+                wire_offset64(wr, r, d0, &tp);
+                const double g0 = d0[0] * T[0] + d0[1] * T[1] + d0[2] * T[2];
+                if (!(g0 <= 0.0)) continue;
+                wire_offset64(wr, rn, d1, &tp);
+                const double g1 = d1[0] * Tn[0] + d1[1] * Tn[1] + d1[2] * Tn[2];
+                if (!(g1 > 0.0)) continue;
+                const double tau = g0 / (g0 - g1);
+                double P[3], d[3];
+#pragma unroll
+                for (int i = 0; i < 3; ++i) P[i] = r[i] + tau * (rn[i] - r[i]);
+                wire_offset64(wr, P, d, &tp);
+                const double D = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+                const double zw = tp * (double)wr[4];
+                const double resid = D - (double)drift[w];
+                if (fabs(zw) <= A.g.z_half && resid * resid < A.lambda) {
+                    n_match += 1;
+                    chi2 += resid * resid;
+                    if (wire_label) {               // C12: smallest |resid| wins, ties -> earliest
+                        const double ad = fabs(resid);
+                        if (wire_label[w] < 0 || ad < wire_best[w]) { wire_label[w] = turn; wire_best[w] = ad; }
+                    }
+                }
+            }
+            m += 1;
+        }
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { r[i] = rn[i]; T[i] = Tn[i]; }
+        n += 1;
+        p = p0 - A.eloss_h * (double)m;                                 // C6
+        const bool cnext = r[0] * r[0] + r[1] * r[1] >= A.g.R0 * A.g.R0;
+        if (!cn && cnext) turn += 1;                                    // C7
+        cn = cnext;
+        if (fabs(r[2]) > A.g.z_half) break;
+        if (r[0] * r[0] + r[1] * r[1] > A.g.r_out * A.g.r_out) break;
+        if (!(p > 1.0)) break;
+        if (!(isfinite(r[0]) && isfinite(r[1]) && isfinite(r[2]) && isfinite(T[0]) && isfinite(T[1]) && isfinite(T[2])))
+            break;
+    }
+    out.n_match = n_match; out.chi2 = chi2; out.n_steps = n; out.turns = turn; out.m_gas = m;
+}
+
+__device__ __forceinline__ uint32_t pool_size(const unsigned long long *counters, uint32_t cap)
+{
+    const unsigned long long c = counters[CNT_POOL];
+    return (uint32_t)(c < (unsigned long long)cap ? c : (unsigned long long)cap);
+}
+
+__device__ __forceinline__ bool qualifies(const PoolEntry &pe, const uint64_t *best_key, float margin)
+{
+    const float Smax = __uint_as_float((uint32_t)(best_key[pe.event] >> 32));
+    return pe.S32 >= Smax - margin;
+}
+
+// one thread per pool entry: fp64 score of the entries within the margin of the final fp32 maximum
+__global__ void rescore_kernel(const BestArgs A, const PoolEntry *pool, uint32_t pool_cap,
+                               const unsigned long long *counters, const uint64_t *best_key, float margin,
+                               double *pool_S64, double *pool_chi2, int32_t *pool_nmatch,
+                               unsigned long long *ev_maxS)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= pool_size(counters, pool_cap)) return;
+    const PoolEntry pe = pool[i];
+    if (!qualifies(pe, best_key, margin)) { pool_S64[i] = -1.0; return; }
+    Eval64 ev;
+    eval_seed64(A, (int)pe.event, pe.index, ev, nullptr, nullptr);
+    const double S = (double)ev.n_match - ev.chi2 / A.lambda;           // C10
+    pool_S64[i] = S; pool_chi2[i] = ev.chi2; pool_nmatch[i] = ev.n_match;
+    atomicMax(ev_maxS + pe.event, (unsigned long long)__double_as_longlong(S > 0.0 ? S : 0.0));
+}
+
+// ties -> lowest linear index
+__global__ void pick_kernel(const PoolEntry *pool, uint32_t pool_cap, const unsigned long long *counters,
+                            const double *pool_S64, const unsigned long long *ev_maxS, unsigned long long *ev_best)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= pool_size(counters, pool_cap)) return;
+    const double S = pool_S64[i];
+    if (S < 0.0) return;
+    const PoolEntry pe = pool[i];
+    if ((unsigned long long)__double_as_longlong(S) == ev_maxS[pe.event]) atomicMin(ev_best + pe.event, (unsigned long long)pe.index);
+}
+
+// one thread per event: re-propagate the best seed, label wires, report (index, n_match, chi2)
+__global__ void label_kernel(const BestArgs A, int n_events, const unsigned long long *ev_best, int32_t *wire_label,
+                             double *wire_best, int64_t *best_seed, uint32_t *best_n_match, double *best_chi2)
+{
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n_events) return;
+    const unsigned long long b = ev_best[e];
+    if (b == ~0ull) {                      // no candidate survived (pool overflow): report "none"
+        best_seed[e] = -1; best_n_match[e] = 0; best_chi2[e] = 0.0;
+        return;
+    }
+    Eval64 ev;
+    eval_seed64(A, e, (uint32_t)b, ev, wire_label + (size_t)e * A.W, wire_best + (size_t)e * A.W);
+    best_seed[e] = (int64_t)b; best_n_match[e] = (uint32_t)ev.n_match; best_chi2[e] = ev.chi2;
+}
+
+__global__ void fill_i32(int32_t *p, size_t n, int32_t v)
+{
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = v;
+}
+
+__global__ void gather_labels(int32_t W, const int32_t *offsets, const int32_t *wire_id, const int32_t *wire_label,
+                              int32_t *labels)
+{
+    const int e = blockIdx.y;
+    const int i = offsets[e] + blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= offsets[e + 1]) return;
+    labels[i] = wire_label[(size_t)e * W + wire_id[i]];
+}
+
+}  // namespace
+
+cudaError_t launch_best_track(const BestLaunch &L, cudaStream_t s)
+{
+    BestArgs A;
+    A.g = L.g; A.grids = L.d_grids; A.axes = L.d_axes; A.axis_stride = L.axis_stride;
+    A.drift_tab = L.d_drift_tab; A.bits = L.d_bits; A.W = L.W; A.n_bit_words = L.n_bit_words;
+    A.h = L.h; A.lambda = L.window * L.window; A.eloss_h = L.eloss * L.h; A.kq = CDC_KAPPA * (double)L.charge;
+    A.max_steps = L.max_steps;
+    cudaError_t e;
+    if ((e = cudaMemsetAsync(L.d_ev_maxS, 0, sizeof(unsigned long long) * (size_t)L.n_events, s)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(L.d_ev_best, 0xFF, sizeof(unsigned long long) * (size_t)L.n_events, s)) != cudaSuccess) return e;
+    const unsigned nb = (L.pool_cap + 63) / 64;
+    rescore_kernel<<<nb, 64, 0, s>>>(A, L.d_pool, L.pool_cap, L.d_counters, L.d_best_key, L.margin, L.d_pool_S64,
+                                     L.d_pool_chi2, L.d_pool_nmatch, L.d_ev_maxS);
+    pick_kernel<<<nb, 64, 0, s>>>(L.d_pool, L.pool_cap, L.d_counters, L.d_pool_S64, L.d_ev_maxS, L.d_ev_best);
+    const size_t nw = (size_t)L.n_events * L.W;
+    fill_i32<<<(unsigned)((nw + 255) / 256), 256, 0, s>>>(L.d_wire_label, nw, -1);
+    label_kernel<<<(L.n_events + 31) / 32, 32, 0, s>>>(A, L.n_events, L.d_ev_best, L.d_wire_label, L.d_wire_best,
+                                                         L.d_best_seed, L.d_best_n_match, L.d_best_chi2);
+    if (L.max_hits_per_event > 0 && L.d_labels) {
+        dim3 grid((unsigned)((L.max_hits_per_event + 127) / 128), (unsigned)L.n_events);
+        gather_labels<<<grid, 128, 0, s>>>(L.W, L.d_offsets, L.d_wire_id, L.d_wire_label, L.d_labels);
+    }
+    return cudaGetLastError();
+}

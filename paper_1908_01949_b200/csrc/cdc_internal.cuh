@@ -1,0 +1,206 @@
+// Internal declarations shared by the translation units of libcdc_seedscan.so.
+// Nothing here is visible through the C ABI (include/cdc_seedscan.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/cdc_seedscan.h"
+
+#define CDC_MAX_LAYERS 32
+#define CDC_KAPPA 0.299792458   // curvature [1/mm] = kappa q B[T] / p[MeV/c]  (reading C1)
+#define CDC_MAX_AXIS 4096
+
+// ---- device-side tables (A0) -------------------------------------------------------------------
+struct LayerDev {            // 32 B, one per sense layer, read through shared memory in the scan
+    float r;                 // waist radius
+    float shift_k;           // sigma_j tan|eps| / r_j : azimuth shift of the wire at height z is atan(z * shift_k)
+    float phi0;
+    float kscale;            // n_j / 2 pi
+    float uz;                // cos(eps) as stored in the canonical wire table
+    float inv_uz;
+    int32_t n;
+    int32_t offset;
+};
+
+struct FieldDev {
+    int32_t kind;
+    float bz;                // uniform field
+    int32_t nr, nz;
+    float r0, z0, inv_dr, inv_dz;
+    const float2 *tab;       // [nz][nr] (B_r, B_z)
+};
+
+struct GeomDev {
+    int32_t n_layers, n_wires_total, n_bit_words;
+    float r_first, inv_pitch, tan_abs;       // layer lookup: j = (u - r_first) * inv_pitch, u^2 = rho^2 - (z tan)^2
+    float u2_lo, u2_hi;                      // lookup is skipped outside this band of u^2
+    float R0sq, z_half, r_out_sq;
+    const float4 *wire4;                     // (w0x, w0y, ux, uy)
+    const LayerDev *layers;                  // device copy
+};
+
+// fp64 view for the exact re-score (A8/A9)
+struct Geom64 {
+    int32_t n_layers, n_wires_total;
+    double R0, z_half, r_out;
+    const float *wire5;                      // canonical [W][5]
+    const LayerDev *layers;
+    float r_first, inv_pitch, tan_abs;
+    int32_t field_kind;
+    double bz;
+    int32_t nr, nz;
+    double r0, z0, dr, dz;
+    const float *tab;                        // [nz][nr][2]
+};
+
+struct cdc_geometry {
+    int32_t n_layers = 0, W = 0;
+    std::vector<double> r, phi0, stereo;
+    std::vector<int32_t> n_wires, offset;
+    std::vector<float> wire5;
+    double z_half = 0, R0 = 0, r_out = 0;
+    cdc_field_desc field{};                  // h_br_bz replaced by field_tab.data()
+    std::vector<float> field_tab;
+    // device
+    float4 *d_wire4 = nullptr;
+    float *d_wire5 = nullptr;
+    float2 *d_field = nullptr;
+    LayerDev *d_layers = nullptr;
+    GeomDev gd{};
+    FieldDev fd{};
+    Geom64 g64{};
+};
+
+struct PoolEntry {           // one rescoring candidate (reading C11)
+    uint32_t event;
+    uint32_t index;          // linear seed index within the event's grid
+    float S32;
+    uint32_t pad;
+};
+
+struct AxisTables {          // per event, device: seed-axis node values in fp64 (A3)
+    // layout [n_events][6][stride]: R0 cos(theta), R0 sin(theta), z, px, py, pz
+    double *d = nullptr;
+    int32_t stride = 0;
+};
+
+struct GridDev {             // per event, passed in a device array
+    int32_t n[5];
+    int32_t n_seeds;
+    int64_t out_offset;      // offset of this event's seeds in the concatenated per-seed outputs
+};
+
+struct cdc_events {
+    const cdc_geometry *geom = nullptr;
+    int32_t n_events = 0, total_hits = 0, W = 0, n_bit_words = 0;
+    std::vector<int32_t> offsets;
+    int32_t *d_offsets = nullptr, *d_wire_id = nullptr;
+    float *d_drift = nullptr;
+    float *d_drift_tab = nullptr;            // [n_events][W]
+    uint32_t *d_bits = nullptr;              // [n_events][n_bit_words]
+    int32_t *d_err = nullptr;                // validation flags
+    // scan scratch
+    AxisTables axes;
+    GridDev *d_grids = nullptr;
+    std::vector<GridDev> h_grids;
+    PoolEntry *d_pool = nullptr;
+    uint32_t pool_cap = 0;
+    unsigned long long *d_counters = nullptr;   // [8]: steps, gas steps, approach tests, pool count, ...
+    bool scanned = false;
+    // best-track scratch
+    double *d_pool_S64 = nullptr, *d_pool_chi2 = nullptr;
+    int32_t *d_pool_nmatch = nullptr;
+    unsigned long long *d_ev_maxS = nullptr;    // per event: bits of the fp64 maximum
+    unsigned long long *d_ev_best = nullptr;    // per event: lowest index attaining it
+    int32_t *d_wire_label = nullptr;            // [n_events][W] turn label per wire (labels)
+    double *d_wire_best = nullptr;              // [n_events][W] smallest |resid| so far
+    unsigned long long *d_peak_key = nullptr;   // Hough scratch [n_events]
+    int32_t max_hits_per_event = 0;
+};
+
+enum { CNT_STEPS = 0, CNT_GAS = 1, CNT_TESTS = 2, CNT_POOL = 3, CNT_N = 8 };
+
+// ---- error plumbing ------------------------------------------------------------------------------
+void cdc_set_error(const std::string &msg);
+#define CDC_FAIL(code, msg) do { cdc_set_error(msg); return (code); } while (0)
+#define CDC_CUDA(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { \
+    cdc_set_error(std::string(#expr) + ": " + cudaGetErrorString(e_)); \
+    return (e_ == cudaErrorMemoryAllocation) ? CDC_ERR_NOMEM : CDC_ERR_CUDA; } } while (0)
+
+// ---- launchers implemented in the kernel translation units ---------------------------------------
+struct ScanLaunch {
+    GeomDev gd;
+    FieldDev fd;
+    int32_t n_events;
+    const GridDev *d_grids;
+    const double *d_axes;
+    int32_t axis_stride;
+    const float *d_drift_tab;
+    const uint32_t *d_bits;
+    float h, lambda, eloss_h;        // eloss_h = eloss per step (MeV)
+    double h64;
+    int32_t max_steps, charge;
+    float margin;
+    uint32_t *d_n_match;
+    float *d_chi2;
+    cdc_seed_debug *d_debug;
+    uint64_t *d_best_key;
+    PoolEntry *d_pool;
+    uint32_t pool_cap;
+    unsigned long long *d_counters;
+    int64_t max_seeds_per_event;
+};
+cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s);
+
+cudaError_t launch_bin_events(int32_t n_events, int32_t W, int32_t n_bit_words, int32_t max_hits_per_event,
+                              const int32_t *d_offsets, const int32_t *d_wire_id, const float *d_drift,
+                              float *d_drift_tab, uint32_t *d_bits, int32_t *d_err, cudaStream_t s);
+
+struct HoughLaunch {
+    int32_t n_events, nR, ncy, ncx;
+    float bin_xy, bin_R, tol, R_lo, half_xy, origin;
+    double bin_xy64, bin_R64, R_lo64, half_xy64, R0, half_theta, half_pt, bz;
+    int32_t charge;
+    const float *d_wire5;
+    const int32_t *d_offsets, *d_wire_id;
+    const float *d_zref;
+    double *d_ranges;
+    int32_t *d_peak;
+    uint32_t *d_accum;
+    unsigned long long *d_peak_key;     // scratch [n_events]
+};
+cudaError_t launch_hough(const HoughLaunch &L, cudaStream_t s);
+
+struct BestLaunch {
+    Geom64 g;
+    int32_t n_events;
+    const GridDev *d_grids;
+    const double *d_axes;
+    int32_t axis_stride;
+    const int32_t *d_offsets, *d_wire_id;
+    const float *d_drift, *d_drift_tab;
+    const uint32_t *d_bits;
+    int32_t W, n_bit_words, max_hits_per_event;
+    double h, window, eloss;
+    int32_t max_steps, charge;
+    float margin;
+    const uint64_t *d_best_key;
+    const PoolEntry *d_pool;
+    uint32_t pool_cap;
+    const unsigned long long *d_counters;
+    double *d_pool_S64, *d_pool_chi2;
+    int32_t *d_pool_nmatch;
+    unsigned long long *d_ev_maxS, *d_ev_best;
+    int32_t *d_wire_label;
+    double *d_wire_best;
+    int64_t *d_best_seed;
+    uint32_t *d_best_n_match;
+    double *d_best_chi2;
+    int32_t *d_labels;
+};
+cudaError_t launch_best_track(const BestLaunch &L, cudaStream_t s);
+
+cudaError_t run_fp32_peak_probe(int32_t iters, double *flops_per_s, double *ms, cudaStream_t s);

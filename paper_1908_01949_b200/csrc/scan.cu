@@ -1,0 +1,364 @@
+// A3-A7: the RKN propagate-and-score kernel with fused per-event argmax and candidate pool.
+//
+// One thread per seed (BJ north_star); the Nystroem-RK4 state lives in registers.  Arithmetic is fp32
+// FMA chains; the six state components are carried as (hi, lo) pairs with a Kahan-compensated update so
+// that the position after thousands of steps stays within the 1e-3 mm parity bound.
+//
+//   PAPER.md:51      seed (theta0, z0, px0, py0, pz0) at R0                     -> seed_init()
+//   PAPER.md:55      RKN propagation (textbook Nystroem scheme, reading C5)     -> rkn_step()
+//   PAPER.md:55,:69  DCA to fired wires, sign-change ownership (reading C9)     -> score_wire()
+//   PAPER.md:65-69   Eq. (1): S = sum (1 - d^2/lambda) over matched terms       -> end of seed_scan_kernel
+//   PAPER.md:69      lowest E (= highest S) wins                                -> packed-key atomicMax
+#include "cdc_internal.cuh"
+
+namespace {
+
+constexpr int kBlock = 128;
+constexpr int kMaxBitWords = 256;          // 8192 wires
+
+struct ScanArgs {
+    GeomDev gd;
+    FieldDev fd;
+    const GridDev *grids;
+    const double *axes;
+    int32_t axis_stride;
+    const float *drift_tab;
+    const uint32_t *bits;
+    float h, h_half, h2_8, h2_2, h_6, h2_6;
+    double kq;                 // kappa * charge
+    double h6_64;              // h / 6 in fp64 (for the systematic-rounding correction)
+    float lambda, inv_lambda, eloss_h;
+    int32_t max_steps;
+    float margin;
+    uint32_t *n_match;
+    float *chi2;
+    cdc_seed_debug *debug;
+    unsigned long long *best_key;
+    PoolEntry *pool;
+    uint32_t pool_cap;
+    unsigned long long *counters;
+};
+
+// atan2 good to ~2e-5 rad: it only selects candidate cells (a superset with ~7 mm of slack, reading C8).
+__device__ __forceinline__ float coarse_atan2(float y, float x)
+{
+    float ax = fabsf(x), ay = fabsf(y);
+    float mx = fmaxf(ax, ay), mn = fminf(ax, ay);
+    float t = __fdividef(mn, mx);
+    float t2 = t * t;
+    float p = fmaf(t2, -0.0117212f, 0.05265332f);
+    p = fmaf(p, t2, -0.11643287f);
+    p = fmaf(p, t2, 0.19354346f);
+    p = fmaf(p, t2, -0.33262347f);
+    p = fmaf(p, t2, 0.99997726f);
+    p = p * t;
+    if (ay > ax) p = 1.57079637f - p;
+    if (x < 0.0f) p = 3.14159274f - p;
+    return copysignf(p, y);
+}
+
+template <int FIELD>
+__device__ __forceinline__ void field_at(const FieldDev &F, float x, float y, float z, float &Bx, float &By,
+                                         float &Bz)
+{
+    if (FIELD == 0) {
+        Bx = 0.0f; By = 0.0f; Bz = F.bz;
+    } else {
+        float rho2 = fmaf(x, x, y * y);
+        float inv_rho = rho2 > 0.0f ? rsqrtf(rho2) : 0.0f;
+        float rho = rho2 * inv_rho;
+        float fr = (rho - F.r0) * F.inv_dr;
+        float fz = (z - F.z0) * F.inv_dz;
+        int ir = min(max(__float2int_rd(fr), 0), F.nr - 2);
+        int iz = min(max(__float2int_rd(fz), 0), F.nz - 2);
+        float wr = fr - (float)ir, wz = fz - (float)iz;
+        const float2 *p = F.tab + iz * F.nr + ir;
+        float2 n00 = __ldg(p), n01 = __ldg(p + 1), n10 = __ldg(p + F.nr), n11 = __ldg(p + F.nr + 1);
+        float br0 = fmaf(wr, n01.x - n00.x, n00.x), br1 = fmaf(wr, n11.x - n10.x, n10.x);
+        float bz0 = fmaf(wr, n01.y - n00.y, n00.y), bz1 = fmaf(wr, n11.y - n10.y, n10.y);
+        float Br = fmaf(wz, br1 - br0, br0);
+        Bz = fmaf(wz, bz1 - bz0, bz0);
+        float s = Br * inv_rho;
+        Bx = s * x; By = s * y;
+    }
+}
+
+// Kahan-compensated accumulation: (hi, lo) += d, lo holds what the last rounding lost.
+__device__ __forceinline__ void comp_add(float &hi, float &lo, float d)
+{
+    float y = d + lo;
+    float t = hi + y;
+    lo = y - (t - hi);
+    hi = t;
+}
+
+struct Vertex {            // what scoring needs of a step vertex
+    float x, y, z, xl, yl, Tx, Ty, Tz;
+};
+
+// One candidate wire that has a hit: does interval n own an approach to it, and does the hit match?
+__device__ __forceinline__ void score_wire(const ScanArgs &A, const float *drift_e, int w, float uz, float inv_uz, const Vertex &v0,
+                                           const Vertex &v1, uint32_t &nm, float &chi2)
+{
+    float4 wr = __ldg(A.gd.wire4 + w);
+    float zt0 = v0.z * inv_uz;
+    float ex0 = fmaf(-zt0, wr.z, v0.x - wr.x) + v0.xl;     // offset from the wire point at the vertex' height
+    float ey0 = fmaf(-zt0, wr.w, v0.y - wr.y) + v0.yl;
+    float uT0 = fmaf(wr.z, v0.Tx, fmaf(wr.w, v0.Ty, uz * v0.Tz));
+    float eu0 = fmaf(ex0, wr.z, ey0 * wr.w);
+    float g0 = fmaf(ex0, v0.Tx, fmaf(ey0, v0.Ty, -eu0 * uT0));   // g = delta . T, delta = e - (e.u) u
+    if (!(g0 <= 0.0f)) return;
+    float zt1 = v1.z * inv_uz;
+    float ex1 = fmaf(-zt1, wr.z, v1.x - wr.x) + v1.xl;
+    float ey1 = fmaf(-zt1, wr.w, v1.y - wr.y) + v1.yl;
+    float uT1 = fmaf(wr.z, v1.Tx, fmaf(wr.w, v1.Ty, uz * v1.Tz));
+    float eu1 = fmaf(ex1, wr.z, ey1 * wr.w);
+    float g1 = fmaf(ex1, v1.Tx, fmaf(ey1, v1.Ty, -eu1 * uT1));
+    if (!(g1 > 0.0f)) return;
+    float tau = __fdividef(g0, g0 - g1);
+    float ex = fmaf(tau, ex1 - ex0, ex0);                   // e is linear in the position: exact chord point
+    float ey = fmaf(tau, ey1 - ey0, ey0);
+    float eu = fmaf(ex, wr.z, ey * wr.w);
+    float D2 = fmaf(ex, ex, fmaf(ey, ey, -eu * eu));
+    float D = sqrtf(fmaxf(D2, 0.0f));
+    float zP = fmaf(tau, v1.z - v0.z, v0.z);
+    float zw = fmaf(eu, uz, zP);
+    float resid = D - __ldg(drift_e + w);
+    float r2 = resid * resid;
+    if (fabsf(zw) <= A.gd.z_half && r2 < A.lambda) { nm += 1u; chi2 += r2; }
+}
+
+__device__ __forceinline__ void score_layer(const ScanArgs &A, const float *drift_e, const LayerDev *s_layer, const uint32_t *s_bits,
+                                            int j, float phi, const Vertex &v0, const Vertex &v1, uint32_t &nm,
+                                            float &chi2, uint32_t &tests)
+{
+    if ((unsigned)j >= (unsigned)A.gd.n_layers) return;
+    const LayerDev L = s_layer[j];
+    float tau = v0.z * L.shift_k;
+    float sh = fmaf(-0.333333343f * tau * tau, tau, tau);      // atan(tau), |tau| < 0.1
+    float kf = (phi - L.phi0 - sh) * L.kscale;
+    float kn = rintf(kf);
+    int k1 = (int)kn;
+    int k2 = k1 + ((kf - kn) >= 0.0f ? 1 : -1);
+    k1 += (k1 < 0) ? L.n : 0; k1 += (k1 < 0) ? L.n : 0; k1 -= (k1 >= L.n) ? L.n : 0;
+    k2 += (k2 < 0) ? L.n : 0; k2 += (k2 < 0) ? L.n : 0; k2 -= (k2 >= L.n) ? L.n : 0;
+    int w1 = L.offset + k1, w2 = L.offset + k2;
+    if ((s_bits[w1 >> 5] >> (w1 & 31)) & 1u) { tests += 1u; score_wire(A, drift_e, w1, L.uz, L.inv_uz, v0, v1, nm, chi2); }
+    if ((s_bits[w2 >> 5] >> (w2 & 31)) & 1u) { tests += 1u; score_wire(A, drift_e, w2, L.uz, L.inv_uz, v0, v1, nm, chi2); }
+}
+
+__device__ __forceinline__ unsigned long long warp_max_u64(unsigned long long v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        unsigned long long other = __shfl_xor_sync(0xffffffffu, v, o);
+        v = other > v ? other : v;
+    }
+    return v;
+}
+
+template <int FIELD, bool ELOSS>
+__global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
+{
+    __shared__ LayerDev s_layer[CDC_MAX_LAYERS];
+    __shared__ uint32_t s_bits[kMaxBitWords];
+
+    const int e = blockIdx.y;
+    const GridDev G = A.grids[e];
+    if ((int64_t)blockIdx.x * kBlock >= (int64_t)G.n_seeds) return;
+    for (int i = threadIdx.x; i < A.gd.n_layers; i += kBlock) s_layer[i] = A.gd.layers[i];
+    for (int i = threadIdx.x; i < A.gd.n_bit_words; i += kBlock)
+        s_bits[i] = A.bits[(size_t)e * A.gd.n_bit_words + i];
+    __syncthreads();
+    const float *drift_e = A.drift_tab + (size_t)e * A.gd.n_wires_total;
+
+    // ---- A3: thread -> seed.  theta is the lane-fastest axis, then px, py, z, pz: neighbouring lanes then
+    // share (z0, p) and leave the chamber within a few steps of one another.
+    const int t = blockIdx.x * kBlock + threadIdx.x;
+    const bool valid = t < G.n_seeds;
+    int q = valid ? t : 0;
+    const int i_th = q % G.n[0]; q /= G.n[0];
+    const int i_px = q % G.n[2]; q /= G.n[2];
+    const int i_py = q % G.n[3]; q /= G.n[3];
+    const int i_z = q % G.n[1];
+    const int i_pz = q / G.n[1];
+    const uint32_t index = (uint32_t)((((i_th * G.n[1] + i_z) * G.n[2] + i_px) * G.n[3] + i_py) * G.n[4] + i_pz);
+
+    float xh, xl, yh, yl, zh, zl, Txh, Txl, Tyh, Tyl, Tzh, Tzl, a, epsT, p0h, p0l;
+    {
+        const double *ax = A.axes + (size_t)e * 6 * A.axis_stride;
+        double x0 = ax[i_th], y0 = ax[A.axis_stride + i_th], z0 = ax[2 * A.axis_stride + i_z];
+        double px = ax[3 * A.axis_stride + i_px], py = ax[4 * A.axis_stride + i_py], pz = ax[5 * A.axis_stride + i_pz];
+        double p0 = sqrt(px * px + py * py + pz * pz);
+        double tx = px / p0, ty = py / p0, tz = pz / p0;
+        xh = (float)x0; xl = (float)(x0 - (double)xh);
+        yh = (float)y0; yl = (float)(y0 - (double)yh);
+        zh = (float)z0; zl = (float)(z0 - (double)zh);
+        Txh = (float)tx; Txl = (float)(tx - (double)Txh);
+        Tyh = (float)ty; Tyl = (float)(ty - (double)Tyh);
+        Tzh = (float)tz; Tzl = (float)(tz - (double)Tzh);
+        double a64 = A.kq / p0;
+        a = (float)a64;
+        // the fp32 roundings of a and h/6 are the same every step; fold their ratio into the T update
+        epsT = (float)((a64 * A.h6_64) / ((double)a * (double)A.h_6) - 1.0);
+        p0h = (float)p0; p0l = (float)(p0 - (double)p0h);
+    }
+    const bool low_p = !(p0h > 1.0f);                 // p <= 1 MeV/c ends a track after its first step (C7)
+
+    uint32_t nm = 0, tests = 0;
+    float chi2 = 0.0f;
+    int n = 0, m = 0, turn = 0;
+    bool cn = true;                                   // c_0 := true (reading C7)
+    const float h = A.h;
+
+    while (valid && n < A.max_steps) {
+        Vertex v0;
+        v0.x = xh; v0.y = yh; v0.z = zh; v0.xl = xl; v0.yl = yl; v0.Tx = Txh; v0.Ty = Tyh; v0.Tz = Tzh;
+
+        // ---- A4: one Nystroem-RK4 step of r'' = a (r' x B(r))
+        float Bx, By, Bz;
+        field_at<FIELD>(A.fd, xh, yh, zh, Bx, By, Bz);
+        float k1x = a * fmaf(Tyh, Bz, -Tzh * By), k1y = a * fmaf(Tzh, Bx, -Txh * Bz), k1z = a * fmaf(Txh, By, -Tyh * Bx);
+        float Ux = fmaf(A.h_half, k1x, Txh), Uy = fmaf(A.h_half, k1y, Tyh), Uz = fmaf(A.h_half, k1z, Tzh);
+        if (FIELD != 0) {
+            float mx = fmaf(A.h2_8, k1x, fmaf(A.h_half, Txh, xh));
+            float my = fmaf(A.h2_8, k1y, fmaf(A.h_half, Tyh, yh));
+            float mz = fmaf(A.h2_8, k1z, fmaf(A.h_half, Tzh, zh));
+            field_at<FIELD>(A.fd, mx, my, mz, Bx, By, Bz);
+        }
+        float k2x = a * fmaf(Uy, Bz, -Uz * By), k2y = a * fmaf(Uz, Bx, -Ux * Bz), k2z = a * fmaf(Ux, By, -Uy * Bx);
+        Ux = fmaf(A.h_half, k2x, Txh); Uy = fmaf(A.h_half, k2y, Tyh); Uz = fmaf(A.h_half, k2z, Tzh);
+        float k3x = a * fmaf(Uy, Bz, -Uz * By), k3y = a * fmaf(Uz, Bx, -Ux * Bz), k3z = a * fmaf(Ux, By, -Uy * Bx);
+        Ux = fmaf(h, k3x, Txh); Uy = fmaf(h, k3y, Tyh); Uz = fmaf(h, k3z, Tzh);
+        if (FIELD != 0) {
+            float ex = fmaf(A.h2_2, k3x, fmaf(h, Txh, xh));
+            float ey = fmaf(A.h2_2, k3y, fmaf(h, Tyh, yh));
+            float ez = fmaf(A.h2_2, k3z, fmaf(h, Tzh, zh));
+            field_at<FIELD>(A.fd, ex, ey, ez, Bx, By, Bz);
+        }
+        float k4x = a * fmaf(Uy, Bz, -Uz * By), k4y = a * fmaf(Uz, Bx, -Ux * Bz), k4z = a * fmaf(Ux, By, -Uy * Bx);
+
+        float dx = fmaf(A.h2_6, (k1x + k2x) + k3x, h * Txh);
+        float dy = fmaf(A.h2_6, (k1y + k2y) + k3y, h * Tyh);
+        float dz = fmaf(A.h2_6, (k1z + k2z) + k3z, h * Tzh);
+        float dTx = A.h_6 * ((k1x + k4x) + 2.0f * (k2x + k3x));
+        float dTy = A.h_6 * ((k1y + k4y) + 2.0f * (k2y + k3y));
+        float dTz = A.h_6 * ((k1z + k4z) + 2.0f * (k2z + k3z));
+        comp_add(xh, xl, fmaf(h, Txl, dx));            // h * T_lo: the part of T the fp32 stages never saw
+        comp_add(yh, yl, fmaf(h, Tyl, dy));
+        comp_add(zh, zl, fmaf(h, Tzl, dz));
+        comp_add(Txh, Txl, fmaf(dTx, epsT, dTx));
+        comp_add(Tyh, Tyl, fmaf(dTy, epsT, dTy));
+        if (FIELD != 0) comp_add(Tzh, Tzl, fmaf(dTz, epsT, dTz));   // uniform field: k_z == 0, T_z is constant
+
+        // ---- A5/A6: wires near r_n, owned approaches, score (only if the interval starts in the gas)
+        if (cn) {
+            float zeta = v0.z * A.gd.tan_abs;
+            float u2 = fmaf(v0.x, v0.x, fmaf(v0.y, v0.y, -zeta * zeta));
+            if (u2 > A.gd.u2_lo && u2 < A.gd.u2_hi) {
+                Vertex v1;
+                v1.x = xh; v1.y = yh; v1.z = zh; v1.xl = xl; v1.yl = yl; v1.Tx = Txh; v1.Ty = Tyh; v1.Tz = Tzh;
+                float u = u2 * rsqrtf(u2);
+                float fj = (u - A.gd.r_first) * A.gd.inv_pitch;
+                float jn = rintf(fj);
+                int jc = (int)jn;
+                int j2 = jc + ((fj - jn) >= 0.0f ? 1 : -1);
+                float phi = coarse_atan2(v0.y, v0.x);
+                score_layer(A, drift_e, s_layer, s_bits, jc, phi, v0, v1, nm, chi2, tests);
+                score_layer(A, drift_e, s_layer, s_bits, j2, phi, v0, v1, nm, chi2, tests);
+            }
+            m += 1;
+        }
+
+        // ---- advance, energy loss (reading C6), turn counter and termination (reading C7)
+        n += 1;
+        float rho2 = fmaf(xh, xh, yh * yh);
+        bool cnext = rho2 >= A.gd.R0sq;
+        if (!cn && cnext) turn += 1;
+        cn = cnext;
+        if (ELOSS) {
+            float p = fmaf(-A.eloss_h, (float)m, p0h) + p0l;
+            a = (float)A.kq / p;      // IEEE division
+            if (!(p > 1.0f)) break;
+        }
+        if (!(fabsf(zh) <= A.gd.z_half)) break;
+        if (!(rho2 <= A.gd.r_out_sq)) break;
+        if (low_p) break;
+    }
+
+    // ---- A7: per-seed output, per-event argmax, candidate pool
+    const float S = valid ? fmaf(-chi2, A.inv_lambda, (float)nm) : -1.0f;
+    if (valid) {
+        const int64_t o = G.out_offset + (int64_t)index;
+        if (A.n_match) A.n_match[o] = nm;
+        if (A.chi2) A.chi2[o] = chi2;
+        if (A.debug) {
+            cdc_seed_debug d;
+            d.n_steps = n; d.turns = turn; d.m_gas = m; d.pad = 0;
+            d.x = (double)xh + (double)xl; d.y = (double)yh + (double)yl; d.z = (double)zh + (double)zl;
+            A.debug[o] = d;
+        }
+    }
+    const float Sc = fmaxf(S, 0.0f);                  // S >= 0 by construction; clamp rounding residue
+    unsigned long long key = valid ? (((unsigned long long)__float_as_uint(Sc) << 32) | (0xFFFFFFFFu - index)) : 0ull;
+    unsigned long long wkey = warp_max_u64(key);
+    const int lane = threadIdx.x & 31;
+    unsigned long long run = 0ull;
+    if (lane == 0) {
+        unsigned long long old = atomicMax(A.best_key + e, wkey);
+        run = old > wkey ? old : wkey;
+    }
+    run = __shfl_sync(0xffffffffu, run, 0);
+    const float S_run = __uint_as_float((uint32_t)(run >> 32));
+    const bool cand = valid && (Sc >= S_run - A.margin);
+    const unsigned ballot = __ballot_sync(0xffffffffu, cand);
+    if (ballot) {
+        unsigned base = 0;
+        if (lane == 0) base = (unsigned)atomicAdd(A.counters + CNT_POOL, (unsigned long long)__popc(ballot));
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (cand) {
+            unsigned pos = base + __popc(ballot & ((1u << lane) - 1u));
+            if (pos < A.pool_cap) {
+                PoolEntry pe; pe.event = (uint32_t)e; pe.index = index; pe.S32 = Sc; pe.pad = 0;
+                A.pool[pos] = pe;
+            }
+        }
+    }
+    unsigned sn = __reduce_add_sync(0xffffffffu, valid ? (unsigned)n : 0u);
+    unsigned sm = __reduce_add_sync(0xffffffffu, valid ? (unsigned)m : 0u);
+    unsigned st = __reduce_add_sync(0xffffffffu, tests);
+    if (lane == 0) {
+        atomicAdd(A.counters + CNT_STEPS, (unsigned long long)sn);
+        atomicAdd(A.counters + CNT_GAS, (unsigned long long)sm);
+        atomicAdd(A.counters + CNT_TESTS, (unsigned long long)st);
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s)
+{
+    ScanArgs A;
+    A.gd = L.gd; A.fd = L.fd; A.grids = L.d_grids; A.axes = L.d_axes; A.axis_stride = L.axis_stride;
+    A.drift_tab = L.d_drift_tab; A.bits = L.d_bits;
+    const double h = L.h64;
+    A.h = (float)h; A.h_half = (float)(h / 2.0); A.h2_8 = (float)(h * h / 8.0); A.h2_2 = (float)(h * h / 2.0);
+    A.h_6 = (float)(h / 6.0); A.h2_6 = (float)(h * h / 6.0);
+    A.kq = CDC_KAPPA * (double)L.charge; A.h6_64 = h / 6.0;
+    A.lambda = L.lambda; A.inv_lambda = 1.0f / L.lambda; A.eloss_h = L.eloss_h;
+    A.max_steps = L.max_steps; A.margin = L.margin;
+    A.n_match = L.d_n_match; A.chi2 = L.d_chi2; A.debug = L.d_debug;
+    A.best_key = (unsigned long long *)L.d_best_key;
+    A.pool = L.d_pool; A.pool_cap = L.pool_cap; A.counters = L.d_counters;
+    if (L.gd.n_bit_words > kMaxBitWords || L.gd.n_layers > CDC_MAX_LAYERS) return cudaErrorInvalidValue;
+    dim3 grid((unsigned)((L.max_seeds_per_event + kBlock - 1) / kBlock), (unsigned)L.n_events);
+    const bool eloss = L.eloss_h != 0.0f;
+    if (L.fd.kind == 0) {
+        if (eloss) seed_scan_kernel<0, true><<<grid, kBlock, 0, s>>>(A);
+        else seed_scan_kernel<0, false><<<grid, kBlock, 0, s>>>(A);
+    } else {
+        if (eloss) seed_scan_kernel<1, true><<<grid, kBlock, 0, s>>>(A);
+        else seed_scan_kernel<1, false><<<grid, kBlock, 0, s>>>(A);
+    }
+    return cudaGetLastError();
+}
