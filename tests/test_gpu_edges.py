@@ -1,0 +1,175 @@
+"""GPU tests of the boundary's remaining calls and of the degenerate cases: A1 tables, error reporting,
+empty / ragged / single-seed inputs, the wire-table builder, device-resident hits, the end-to-end host call."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1908_01949_b200 import api, binding as B, synth
+
+import parity_util as U
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def setup():
+    import torch
+    assert torch.cuda.is_available()
+    cfg, geom, field, events, grids = U.make_workload(1, n_events=3, grid_n=4)
+    return cfg, geom, field, events, grids, api.SeedScanner(geom, field)
+
+
+def test_event_tables_equal_oracle_binning(setup):
+    cfg, geom, field, events, grids, sc = setup
+    off, w, d = synth.pack_hits(events)
+    rng = np.random.default_rng(1)
+    perm = np.concatenate([off[e] + rng.permutation(off[e + 1] - off[e]) for e in range(len(events))])
+    E = sc.upload(off, w[perm], d[perm])                       # hits need not be sorted
+    tab, bits = E.tables()
+    bound = oracle.Bound(geom, field, U.oracle_params(cfg))
+    for e, ev in enumerate(events):
+        assert np.array_equal(tab[e], oracle.bin_event(bound, ev.wire_id, ev.drift_mm))
+        want = np.zeros(bits.shape[1] * 32, dtype=bool); want[ev.wire_id] = True
+        got = ((bits[e][:, None] >> np.arange(32, dtype=np.uint32)[None, :]) & 1).astype(bool).ravel()
+        assert np.array_equal(got, want)
+
+
+def test_upload_errors_are_reported(setup):
+    cfg, geom, field, events, grids, sc = setup
+    off = np.array([0, 3], dtype=np.int32)
+    with pytest.raises(B.CdcError) as ei:
+        sc.upload(off, np.array([1, 2, geom.n_wires_total], dtype=np.int32), np.ones(3, dtype=np.float32))
+    assert ei.value.status == -2
+    with pytest.raises(B.CdcError) as ei:
+        sc.upload(off, np.array([1, 2, 2], dtype=np.int32), np.ones(3, dtype=np.float32))
+    assert ei.value.status == -1 and "duplicate" in str(ei.value)
+    for bad in (-0.5, np.nan, np.inf):
+        with pytest.raises(B.CdcError) as ei:
+            sc.upload(off, np.array([1, 2, 3], dtype=np.int32), np.array([1.0, bad, 1.0], dtype=np.float32))
+        assert ei.value.status == -1
+    E = sc.upload(off, np.array([1, 2, 3], dtype=np.int32), np.ones(3, dtype=np.float32))
+    g = synth.truth_anchored_grid(events[0].seed, 2)[0]
+    import torch
+    key = torch.zeros(1, dtype=torch.int64, device="cuda")
+    with pytest.raises(B.CdcError):
+        B.cdc_seed_scan(sc.geometry, E, B.grid_specs([g]), B.scan_params(0.0, 100), key)       # h <= 0
+    g.n[0] = 0
+    with pytest.raises(B.CdcError):
+        B.cdc_seed_scan(sc.geometry, E, B.grid_specs([g]), B.scan_params(2.0, 100), key)       # n < 1
+    with pytest.raises(B.CdcError) as ei:                                                        # call order
+        B.cdc_best_track(sc.geometry, E, B.grid_specs([g]), B.scan_params(2.0, 100), key, key, key, key, key)
+    assert ei.value.status == -5
+
+
+def test_field_table_too_small_is_rejected(setup):
+    cfg, geom, *_ = setup
+    small = synth.make_table_field(r_max=800.0)
+    with pytest.raises(B.CdcError) as ei:
+        api.SeedScanner(geom, small)
+    assert ei.value.status == -2
+
+
+def test_empty_event_and_ragged_grid(setup):
+    cfg, geom, field, events, grids, sc = setup
+    ev = events[0]
+    # event 0 has no hits at all; event 1 is a real one with a ragged 5 x 3 x 7 x 2 x 3 grid (630 seeds: 4 full
+    # blocks of 128 and a tail of 118)
+    g_empty = synth.truth_anchored_grid(ev.seed, [2, 3, 1, 2, 2])[0]
+    g_rag = synth.truth_anchored_grid(ev.seed, [5, 3, 7, 2, 3])[0]
+    off = np.array([0, 0, ev.wire_id.size], dtype=np.int32)
+    E = sc.upload(off, ev.wire_id, ev.drift_mm)
+    gpu = sc.scan(E, [g_empty, g_rag], U.gpu_params(cfg), per_seed=True, debug=True)
+    n0 = g_empty.n_seeds
+    assert gpu["n_seeds"] == [n0, 630]
+    assert not gpu["n_match"][:n0].any() and not gpu["chi2"][:n0].any()
+    assert gpu["best_seed"][0] == 0 and gpu["best_n_match"][0] == 0 and gpu["best_chi2"][0] == 0.0   # ties -> index 0
+    assert (gpu["debug"]["n_steps"][:n0] > 0).all()
+    orc = oracle.scan_parallel(geom, field, U.oracle_params(cfg), ev.wire_id, ev.drift_mm, g_rag)
+    U.compare_scan(cfg, geom, field, ev, g_rag, gpu, orc, np.arange(630), offset=n0)
+    U.check_best(cfg, geom, field, ev, g_rag, gpu, e=1, orc_full=orc)
+    assert gpu["labels"].size == ev.wire_id.size
+
+
+def test_single_seed_and_step_cap(setup):
+    cfg, geom, field, events, grids, sc = setup
+    ev = events[1]
+    g1 = synth.truth_anchored_grid(ev.seed, 1)[0]
+    off, w, d = synth.pack_hits([ev])
+    E = sc.upload(off, w, d)
+    for cap in (1, 37, cfg.max_steps):
+        gpu = sc.scan(E, [g1], B.scan_params(cfg.h_mm, cap, cfg.window_mm), per_seed=True, debug=True)
+        bound = oracle.Bound(geom, field, dict(h=cfg.h_mm, max_steps=cap, window=cfg.window_mm))
+        r = oracle.eval_seed(bound, ev.wire_id, ev.drift_mm, ev.seed)
+        assert gpu["debug"]["n_steps"][0] == r["n_steps"] == min(cap, r["n_steps"])
+        assert gpu["n_match"][0] == r["n_match"] and gpu["best_seed"][0] == 0
+        assert gpu["best_chi2"][0] == r["chi2"]
+        assert np.linalg.norm([gpu["debug"][k][0] - r["r"][i] for i, k in enumerate("xyz")]) < U.POS_TOL_MM
+
+
+def test_degenerate_seeds_terminate(setup):
+    """Inward-pointing, stiff and very soft seeds are propagated like any other (reading C4) and end by the same rule."""
+    cfg, geom, field, events, grids, sc = setup
+    ev = events[0]
+    off, w, d = synth.pack_hits([ev])
+    E = sc.upload(off, w, d)
+    bound = oracle.Bound(geom, field, U.oracle_params(cfg))
+    for seed in ([0.3, 0.0, -80.0, -30.0, 20.0], [0.0, 0.0, 400.0, 0.0, 1.0], [1.0, 700.0, 0.3, 0.2, 0.5],
+                 [2.0, -749.9, 10.0, 10.0, -50.0]):
+        g = synth.Grid(lo=np.array(seed, dtype=np.float64), step=np.zeros(5), n=np.ones(5, dtype=np.int32))
+        gpu = sc.scan(E, [g], U.gpu_params(cfg), per_seed=True, debug=True)
+        r = oracle.eval_seed(bound, ev.wire_id, ev.drift_mm, np.array(seed))
+        assert gpu["debug"]["n_steps"][0] == r["n_steps"], seed
+        assert gpu["n_match"][0] == r["n_match"]
+
+
+def test_wire_table_builder_matches_generator(setup):
+    cfg, geom, field, *_ = setup
+    sc2 = api.SeedScanner(geom, field, use_wire_table=False)
+    built = sc2.geometry.wire_table()
+    ulp = np.spacing(np.abs(geom.wire).astype(np.float32))
+    assert np.all(np.abs(built - geom.wire) <= ulp)          # same fp64 formula, rounded once: <= 1 ulp (libm vs numpy)
+    assert (built == geom.wire).mean() > 0.999
+    assert np.array_equal(api.SeedScanner(geom, field).geometry.wire_table(), geom.wire)
+
+
+def test_device_resident_hits_and_host_call_agree(setup):
+    import torch
+    cfg, geom, field, events, grids, sc = setup
+    off, w, d = synth.pack_hits(events)
+    E_host = sc.upload(off, w, d)
+    E_dev = sc.upload(off, torch.tensor(w, device="cuda"), torch.tensor(d, device="cuda"))
+    P = U.gpu_params(cfg)
+    a = sc.scan(E_host, grids, P, per_seed=True)
+    b = sc.scan(E_dev, grids, P, per_seed=True)
+    c = sc.find_tracks_host(off, w, d, grids, P)
+    for k in ("best_seed", "best_n_match", "best_chi2", "labels", "best_key"):
+        assert np.array_equal(a[k], b[k]) and np.array_equal(a[k], c[k]), k
+    assert np.array_equal(a["n_match"], b["n_match"]) and np.array_equal(a["chi2"], b["chi2"])   # deterministic
+    for e, (ev, grid) in enumerate(zip(events, grids)):
+        orc = oracle.scan_parallel(geom, field, U.oracle_params(cfg), ev.wire_id, ev.drift_mm, grid)
+        U.check_best(cfg, geom, field, ev, grid, a, e=e, hit_slice=slice(off[e], off[e + 1]), orc_full=orc)
+
+
+def test_host_call_with_hough_ranges(setup):
+    cfg2, geom, field, events, _ = U.make_workload(2, grid_n=6)
+    sc = api.SeedScanner(geom, field)
+    ev = events[0]
+    off, w, d = synth.pack_hits(events)
+    g0 = synth.truth_anchored_grid(ev.seed, 6)[0]
+    P = U.gpu_params(cfg2)
+    out = sc.find_tracks_host(off, w, d, [g0], P, hp=B.hough_params(), zref=[float(ev.seed[1])])
+    E = sc.upload(off, w, d)
+    h = sc.hough(E, [float(ev.seed[1])])
+    assert np.array_equal(out["ranges"], h["ranges"])
+    lo = g0.lo.copy(); hi = g0.lo + g0.step * (g0.n - 1)
+    lo[[0, 2, 3]] = h["ranges"][0][:, 0]; hi[[0, 2, 3]] = h["ranges"][0][:, 1]
+    grid = synth.ranges_grid(lo, hi, 6)
+    staged = sc.scan(E, [grid], P, per_seed=True)
+    for k in ("best_seed", "best_n_match", "best_chi2", "labels"):
+        assert np.array_equal(out[k], staged[k]), k
+    U.check_best(cfg2, geom, field, ev, grid, staged)
+
+
+def test_fp32_peak_probe_is_near_nominal():
+    f, ms = B.cdc_fp32_peak_probe(2048)
+    assert 40e12 < f < 80e12 and ms > 0

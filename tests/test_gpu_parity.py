@@ -1,0 +1,169 @@
+"""GPU parity tests proper: the CUDA path, called through the C ABI, against the fp64 CPU oracle on the same
+seeded inputs (BASELINE.json north_star tolerances, see parity_util.py).  Run with -m gpu on a B200."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1908_01949_b200 import api, binding as B, synth
+
+import parity_util as U
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "the parity tests need a CUDA device"
+    return torch
+
+
+def _scan_all(sc, events, grids, cfg, **kw):
+    off, w, d = synth.pack_hits(events)
+    E = sc.upload(off, w, d)
+    return sc.scan(E, grids, U.gpu_params(cfg), per_seed=True, debug=True, **kw), off
+
+
+# ------------------------------------------------------------------ config 0: every seed of the grid
+def test_cfg0_full_grid_every_seed(torch_cuda):
+    cfg, geom, field, events, grids = U.make_workload(0, n_events=2)
+    sc = api.SeedScanner(geom, field)
+    gpu, off = _scan_all(sc, events, grids, cfg)
+    listed = 0
+    for e, (ev, grid) in enumerate(zip(events, grids)):
+        orc = oracle.scan_parallel(geom, field, U.oracle_params(cfg), ev.wire_id, ev.drift_mm, grid)
+        sel = np.arange(grid.n_seeds)
+        o = e * grid.n_seeds
+        listed += len(U.compare_scan(cfg, geom, field, ev, grid, gpu, orc, sel, offset=o))
+        U.check_best(cfg, geom, field, ev, grid, gpu, e=e, hit_slice=slice(off[e], off[e + 1]), orc_full=orc)
+        # fused fp32 argmax agrees with the fp32 per-seed outputs it was reduced from
+        S32 = gpu["n_match"][o:o + grid.n_seeds].astype(np.float32) - gpu["chi2"][o:o + grid.n_seeds]
+        assert abs(float(gpu["S32_max"][e]) - float(S32.max())) < 1e-5
+    st = gpu["stats"]
+    assert st["n_seeds"] == 2 * 8 ** 5 and st["n_pool"] <= st["pool_cap"]
+    assert st["n_steps"] == int(gpu["debug"]["n_steps"].sum())
+    print(f"cfg0: {listed} listed threshold exceptions of {st['n_seeds']} seeds")
+
+
+# ------------------------------------------------------------------ config 1: full size, sampled
+def test_cfg1_full_size_sampled(torch_cuda):
+    cfg, geom, field, events, grids = U.make_workload(1)
+    ev, grid = events[0], grids[0]
+    assert grid.n_seeds == 16 ** 5 and cfg.max_steps == 3000
+    sc = api.SeedScanner(geom, field)
+    gpu, off = _scan_all(sc, events, grids, cfg)
+    sel = synth.stratified_seed_sample(grid.n_seeds, 3000, key=11)
+    orc = oracle.scan_parallel(geom, field, U.oracle_params(cfg), ev.wire_id, ev.drift_mm, grid, index_list=sel)
+    listed = U.compare_scan(cfg, geom, field, ev, grid, gpu, orc, sel)
+    U.check_best(cfg, geom, field, ev, grid, gpu)
+    assert set(gpu["labels"].tolist()) >= {0, 1}          # a double-turn event: both partitions labelled
+    print(f"cfg1: {len(listed)} listed threshold exceptions of {sel.size} sampled seeds")
+
+
+# ------------------------------------------------------------------ config 2: Hough ranges, energy loss, 24^5
+def _hough_edge_votes(geom, ev, zref, hp, bins):
+    """Number of (hit, bin) pairs whose vote is within EDGE_TOL of the tolerance edge, for the listed bins."""
+    w = geom.wire[ev.wire_id].astype(np.float64)
+    t = zref / w[:, 4]
+    x, y = w[:, 0] + t * w[:, 2], w[:, 1] + t * w[:, 3]
+    n = 0
+    for (iR, icy, icx) in bins:
+        R = hp["R_lo_mm"] + (iR + 0.5) * hp["bin_R_mm"]
+        cy = -hp["half_xy_mm"] + (icy + 0.5) * hp["bin_xy_mm"]
+        cx = -hp["half_xy_mm"] + (icx + 0.5) * hp["bin_xy_mm"]
+        d = np.hypot(cx - x, cy - y)
+        edge = np.abs(np.abs(d - R) - hp["tol_mm"]) < U.EDGE_TOL_MM
+        elig = abs(math.hypot(cx, cy) - R) - (hp["origin_mm"] + hp["tol_mm"])
+        n += int(edge.sum()) + int(abs(elig) < U.EDGE_TOL_MM)
+    return n
+
+
+def test_cfg2_hough_ranges_eloss_full_size(torch_cuda):
+    cfg, geom, field, events, _ = U.make_workload(2)
+    ev = events[0]
+    assert cfg.eloss_MeV_per_mm > 0 and cfg.max_steps == 4500 and cfg.grid_n == 24
+    sc = api.SeedScanner(geom, field)
+    off, w, d = synth.pack_hits(events)
+    E = sc.upload(off, w, d)
+    zref = float(ev.seed[1])
+    # --- A2 parity: accumulator, peak, ranges
+    h = sc.hough(E, [zref], want_accum=True)
+    bound = oracle.Bound(geom, field, U.oracle_params(cfg))
+    ho = oracle.hough(bound, ev.wire_id, ev.drift_mm, zref=float(np.float32(zref)))
+    acc_g, acc_o = h["accum"][0], ho["accum"]
+    diff = np.argwhere(acc_g != acc_o)
+    assert diff.shape[0] < 200
+    if diff.shape[0]:
+        n_edge = _hough_edge_votes(geom, ev, float(np.float32(zref)), B.HOUGH_DEFAULT, [tuple(x) for x in diff])
+        assert n_edge >= diff.shape[0]                      # every differing bin has an edge vote
+        assert np.abs(acc_g.astype(np.int64) - acc_o.astype(np.int64)).max() <= 2
+    runner_up = np.sort(acc_o.ravel())[-2]
+    if ho["peak"][3] - runner_up > 2 or diff.shape[0] == 0:
+        assert np.array_equal(h["peak"][0], ho["peak"])
+        assert np.allclose(h["ranges"][0], ho["ranges"], rtol=0, atol=1e-9)
+    # --- the scan's grid: (theta, px, py) from the GPU's Hough ranges, (z, pz) truth-anchored
+    g0, _ = synth.truth_anchored_grid(ev.seed, cfg.grid_n)
+    rg = h["ranges"][0]
+    lo = g0.lo.copy(); hi = g0.lo + g0.step * (g0.n - 1)
+    lo[[0, 2, 3]] = rg[:, 0]; hi[[0, 2, 3]] = rg[:, 1]
+    grid = synth.ranges_grid(lo, hi, cfg.grid_n)
+    assert grid.n_seeds == 24 ** 5
+    gpu = sc.scan(E, [grid], U.gpu_params(cfg), per_seed=True, debug=True)
+    sel = synth.stratified_seed_sample(grid.n_seeds, 1500, key=12)
+    orc = oracle.scan_parallel(geom, field, U.oracle_params(cfg), ev.wire_id, ev.drift_mm, grid, index_list=sel)
+    listed = U.compare_scan(cfg, geom, field, ev, grid, gpu, orc, sel)
+    U.check_best(cfg, geom, field, ev, grid, gpu)
+    print(f"cfg2: {len(listed)} listed threshold exceptions of {sel.size}; best S32 {gpu['S32_max'][0]:.3f}")
+
+
+def orc_m_gas(bound, ev, grid, sel):
+    return np.array([oracle.eval_seed(bound, ev.wire_id, ev.drift_mm, grid.node(grid.unravel(int(i))))["m_gas"]
+                     for i in sel])
+
+
+def test_cfg2_in_gas_step_count_drives_energy_loss(torch_cuda):
+    """m_gas (the integer the momentum loss is defined through, reading C6) equals the oracle's."""
+    cfg, geom, field, events, grids = U.make_workload(2, grid_n=6)
+    ev, grid = events[0], grids[0]
+    sc = api.SeedScanner(geom, field)
+    gpu, _ = _scan_all(sc, events, grids, cfg, best=False)
+    bound = oracle.Bound(geom, field, U.oracle_params(cfg))
+    sel = synth.stratified_seed_sample(grid.n_seeds, 300, key=5)
+    m = orc_m_gas(bound, ev, grid, sel)
+    same = gpu["debug"]["m_gas"][sel] == m
+    assert same.mean() > 0.99
+    for i in np.nonzero(~same)[0]:
+        assert U.explain_mismatch(bound, ev, grid.node(grid.unravel(int(sel[i]))), cfg, geom)
+
+
+# ------------------------------------------------------------------ config 3: tabulated field, event batch
+def test_cfg3_table_field_batch(torch_cuda):
+    cfg, geom, field, events, grids = U.make_workload(3, n_events=12)
+    assert field.kind == 1 and {e.n_turns for e in events} >= {1}
+    sc = api.SeedScanner(geom, field)
+    gpu, off = _scan_all(sc, events, grids, cfg)
+    listed = 0
+    for e, (ev, grid) in enumerate(zip(events, grids)):
+        o = e * grid.n_seeds
+        sel = synth.stratified_seed_sample(grid.n_seeds, 250, key=100 + e)
+        orc = oracle.scan_parallel(geom, field, U.oracle_params(cfg), ev.wire_id, ev.drift_mm, grid, index_list=sel)
+        listed += len(U.compare_scan(cfg, geom, field, ev, grid, gpu, orc, sel, offset=o))
+        U.check_best(cfg, geom, field, ev, grid, gpu, e=e, hit_slice=slice(off[e], off[e + 1]))
+    print(f"cfg3: {listed} listed threshold exceptions; turns per event {[e.n_turns for e in events]}")
+
+
+# ------------------------------------------------------------------ config 4: step sizes 1, 2, 4 mm
+@pytest.mark.parametrize("h", [1.0, 4.0])
+def test_cfg4_step_sizes(torch_cuda, h):
+    import dataclasses
+    cfg, geom, field, events, grids = U.make_workload(4, n_events=1, grid_n=8)
+    cfg = dataclasses.replace(cfg, h_mm=h, max_steps=int(9000 / h))
+    ev, grid = events[0], grids[0]
+    sc = api.SeedScanner(geom, field)
+    gpu, _ = _scan_all(sc, events, grids, cfg)
+    sel = synth.stratified_seed_sample(grid.n_seeds, 1200, key=int(h))
+    orc = oracle.scan_parallel(geom, field, U.oracle_params(cfg), ev.wire_id, ev.drift_mm, grid, index_list=sel)
+    U.compare_scan(cfg, geom, field, ev, grid, gpu, orc, sel)
+    U.check_best(cfg, geom, field, ev, grid, gpu)
