@@ -1,0 +1,257 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the CDC seed-scan hot path on B200 (BASELINE.json metric: seed-propagations/s).
+
+A "step" is one pass of the whole hot path over one batch of synthetic events: A1 event binning, A2 Hough
+pre-vote, A3-A7 RKN propagate-and-score with fused argmax, A8 fp64 re-score of the near-best seeds, A9 labels
+(DESIGN.md section 2).  Default workload = BASELINE.json configs[1] (one double-turn event, 10 % noise,
+16^5 = 1,048,576 seeds, <= 3000 steps of 2 mm).  One JSON line on stdout (rank 0).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg0|cfg1|cfg2|cfg3] [--events E] [--grid-n G]
+    python bench.py --impl reference ...     # the CPU oracle on this box's host cores, same metric
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1908_01949_b200 import synth  # noqa: E402
+
+METRIC = "seed_propagations_per_s"
+UNIT = "seeds/s"
+# Algorithmic FP32 flops (FMA = 2) of the scan kernel's arithmetic, DESIGN.md section 7
+FLOPS_STEP = {0: 78.0, 1: 255.0}        # per RKN step, uniform / tabulated field (compensated state included)
+FLOPS_LOOKUP, FLOPS_G, FLOPS_APPROACH = 43.0, 22.0, 35.0
+PEAK_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # 74.4: 148 SMs x 128 FP32 lanes x 2 x 1965 MHz (B200_PROFILING.md)
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg2", "cfg3"])
+    ap.add_argument("--events", type=int, default=0, help="events per GPU (0 = 1, or 16 for cfg3)")
+    ap.add_argument("--grid-n", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def make_workload(args, rank):
+    cfg_id = int(args.workload[3:])
+    cfg = synth.CONFIGS[cfg_id]
+    geom = synth.make_geometry()
+    field = synth.make_uniform_field() if cfg.field_kind == 0 else synth.make_table_field()
+    n_events = args.events or (16 if cfg_id == 3 else 1)
+    events = synth.generate_events(cfg, geom, field, n_events, first_event=rank * n_events)
+    n = args.grid_n or cfg.grid_n
+    grids = [synth.truth_anchored_grid(ev.seed, n)[0] for ev in events]
+    return cfg_id, cfg, geom, field, events, grids
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                pass
+        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 6 for i in range(4) if r[2 + i].lower() == "active"})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def oracle_sample_time(cfg, geom, field, ev, grid, n_sample, key):
+    """Time the oracle, as it stands, single-threaded, on a stratified sample of the workload's seeds."""
+    import oracle
+    sel = synth.stratified_seed_sample(grid.n_seeds, n_sample, key)
+    b = oracle.Bound(geom, field, dict(h=cfg.h_mm, max_steps=cfg.max_steps, window=cfg.window_mm,
+                                       eloss=cfg.eloss_MeV_per_mm))
+    t0 = time.perf_counter()
+    out = oracle.scan(b, ev.wire_id, ev.drift_mm, grid, index_list=sel)
+    dt = time.perf_counter() - t0
+    return sel.size, int(out["n_steps"].sum()), dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg_id, cfg, geom, field, events, grids = make_workload(args, 0)
+    per_step = 4096
+    times, seeds, steps = [], 0, 0
+    for i in range(args.warmup + args.steps):
+        n, st, dt = oracle_sample_time(cfg, geom, field, events[0], grids[0], per_step, key=1000 + i)
+        if i >= args.warmup:
+            times.append(dt); seeds += n; steps += st
+    total = sum(times)
+    val = seeds / total
+    sample = f"{per_step} stratified seeds of event 0 per step ({steps / max(seeds, 1):.0f} RKN steps/seed)"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "seeds_per_event": grids[0].n_seeds, "max_steps": cfg.max_steps,
+                       "h_mm": cfg.h_mm},
+            "rkn_steps_per_s": steps / total,
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1908_01949_b200 import api, binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg_id, cfg, geom, field, events, grids = make_workload(args, rank)
+    sc = api.SeedScanner(geom, field)
+    off, w, d = synth.pack_hits(events)
+    E = len(events)
+    n_seeds = sum(g.n_seeds for g in grids)
+    specs = B.grid_specs(grids)
+    P = B.scan_params(cfg.h_mm, cfg.max_steps, cfg.window_mm, cfg.eloss_MeV_per_mm)
+    hp = B.hough_params()
+    zref = np.array([ev.seed[1] for ev in events], dtype=np.float32)
+    # device-resident inputs and outputs of the device-timed arm
+    d_w = torch.tensor(w, device="cuda"); d_d = torch.tensor(d, device="cuda"); d_zref = torch.tensor(zref, device="cuda")
+    d_ranges = torch.zeros((E, 3, 2), dtype=torch.float64, device="cuda")
+    d_peak = torch.zeros((E, 4), dtype=torch.int32, device="cuda")
+    d_key = torch.zeros(E, dtype=torch.int64, device="cuda"); d_seed = torch.zeros(E, dtype=torch.int64, device="cuda")
+    d_nm = torch.zeros(E, dtype=torch.int32, device="cuda"); d_c2 = torch.zeros(E, dtype=torch.float64, device="cuda")
+    d_lab = torch.zeros(max(int(off[-1]), 1), dtype=torch.int32, device="cuda")
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")       # > 126 MB L2
+    stats = {}
+
+    def step():
+        ev = B.Events(sc.geometry, off, d_w, d_d)                                   # A1
+        B.cdc_hough_seed_ranges(sc.geometry, ev, hp, -1, d_zref, d_ranges, d_peak)  # A2
+        B.cdc_seed_scan(sc.geometry, ev, specs, P, d_key)                           # A3-A7
+        B.cdc_best_track(sc.geometry, ev, specs, P, d_key, d_seed, d_nm, d_c2, d_lab)   # A8-A9
+        return ev
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        flush.fill_(1); step().close()
+    barrier()
+    sampler = ClockSampler(local); sampler.start()
+    l0 = B.cdc_kernel_launch_count()
+    ms, kernel_ms, acc = [], [], {}
+    for _ in range(args.steps):
+        flush.fill_(1)
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(); ev = step(); e1.record(); e1.synchronize()
+        ms.append(e0.elapsed_time(e1))
+        st = B.cdc_scan_get_stats(ev)
+        kernel_ms.append(st["kernel_ms"])
+        for k, v in st.items():
+            acc[k] = acc.get(k, 0) + v
+        ev.close()
+    barrier()
+    launches = B.cdc_kernel_launch_count() - l0
+    clocks = sampler.stop()
+    best = (d_seed.cpu().numpy().tolist(), d_nm.cpu().numpy().tolist())
+
+    # end to end: host buffers through the C ABI, H2D + D2H inside the timed region (wall clock around the call)
+    pin = lambda a: torch.from_numpy(a).pin_memory().numpy()   # noqa: E731
+    h_off, h_w, h_d = off, pin(w), pin(d)
+    sc.find_tracks_host(h_off, h_w, h_d, grids, P, hp=None)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        out = sc.find_tracks_host(h_off, h_w, h_d, grids, P, hp=None)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    assert out["best_seed"].tolist() == best[0]
+    h2d = int(w.nbytes + d.nbytes + off.nbytes + E * 6 * max(int(g.n.max()) for g in grids) * 8)
+    d2h = int(E * (8 + 4 + 8 + 8) + 4 * int(off[-1]))
+
+    total_ms = float(sum(ms))
+    t = torch.tensor([total_ms, e2e_s, float(sum(kernel_ms))], dtype=torch.float64, device="cuda")
+    cnt = torch.tensor([float(n_seeds), float(acc["n_steps"]), float(E)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX); dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
+    total_ms, e2e_s, ksum_ms = t.tolist()
+    seeds_all, steps_all, events_all = cnt.tolist()
+    if rank == 0:
+        K = args.steps
+        flops = FLOPS_STEP[cfg.field_kind] * acc["n_steps"] + FLOPS_LOOKUP * acc["n_lookups"] + \
+            FLOPS_G * (acc["n_approach_tests"] + acc["n_g1"]) + FLOPS_APPROACH * acc["n_approaches"]
+        k_s = sum(kernel_ms) * 1e-3
+        achieved = flops / k_s / 1e12
+        line = {"metric": METRIC, "value": seeds_all * K / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
+                "warmup": args.warmup, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": args.workload, "events_per_gpu": E, "seeds_per_event": grids[0].n_seeds,
+                           "max_steps": cfg.max_steps, "h_mm": cfg.h_mm, "field": "table" if cfg.field_kind else "uniform",
+                           "hits_per_event": int(off[-1]) // E, "l2": "flushed between steps (256 MB write)",
+                           "parallelism": f"dp{world} (events sharded, no collective)"},
+                "rkn_steps_per_s": steps_all / (total_ms * 1e-3), "events_per_s": events_all * K / (total_ms * 1e-3),
+                "scan_kernel_ms": sum(kernel_ms) / K, "scan_kernel_share": ksum_ms / total_ms,
+                "rkn_steps_per_s_kernel": acc["n_steps"] / k_s,
+                "clocks": clocks,
+                "e2e": {"value": seeds_all * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+                "gpu_launches": int(launches),
+                "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s",
+                             "frac": achieved / PEAK_FP32_TFLOPS, "traffic": None, "kernel": "seed_scan_kernel",
+                             "flops_per_rkn_step": flops / max(acc["n_steps"], 1),
+                             "peak_source": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (nominal, B200_PROFILING.md)"}}
+        f, _ = B.cdc_fp32_peak_probe(4096)
+        line["roofline"]["ffma_probe_tflops"] = f / 1e12
+        line["roofline"]["frac_of_probe"] = achieved / (f / 1e12)
+        if not args.no_cpu_baseline:
+            n, st, dt = oracle_sample_time(cfg, geom, field, events[0], grids[0], 32768 if cfg_id < 3 else 65536, key=77)
+            line["cpu_baseline"] = {"value": n / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                    "sample": f"{n} stratified seeds of event 0 ({st} RKN steps, {dt:.1f} s)",
+                                    "rkn_steps_per_s": st / dt}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    run_reference(a) if a.impl == "reference" else run_ours(a)

@@ -109,6 +109,10 @@ typedef struct {
     uint64_t n_approach_tests; /* live candidate wires examined (g evaluated) */
     uint64_t n_pool;           /* candidate-pool entries appended (reading C11) */
     uint64_t pool_cap;
+    uint64_t n_lookups;        /* in-gas steps that fell inside the wire band and ran the layer/cell lookup */
+    uint64_t n_g1;             /* candidates whose far-end g was evaluated (g_n <= 0) */
+    uint64_t n_approaches;     /* owned approaches (g_n <= 0 < g_{n+1}) scored against the window */
+    double kernel_ms;          /* device time of the propagate-and-score kernel alone (CUDA events on `stream`) */
 } cdc_scan_stats;
 
 const char *cdc_last_error(void);
@@ -179,6 +183,9 @@ int32_t cdc_find_tracks_host(const cdc_geometry *g, int32_t n_events, const int3
                              const float *h_zref_mm_or_null, int64_t *h_best_seed, uint32_t *h_best_n_match,
                              double *h_best_chi2, uint64_t *h_best_key, int32_t *h_labels,
                              double *h_ranges_or_null, void *stream);
+
+/* Number of kernels this library has launched in this process so far (bench.py's gpu_launches). */
+uint64_t cdc_kernel_launch_count(void);
 
 /* Register-only FFMA chain: the empirical FP32 peak used as the roofline denominator.  Runs `iters`
  * dependent-chain iterations on every SM, returns achieved FLOP/s (2 per FFMA).  Synchronises. */

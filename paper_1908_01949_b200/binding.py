@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(HERE, "libcdc_seedscan.so")
 EXPORTS = ["cdc_last_error", "cdc_geometry_create", "cdc_geometry_destroy", "cdc_geometry_wire_table",
            "cdc_event_upload", "cdc_events_destroy", "cdc_events_tables", "cdc_hough_dims",
            "cdc_hough_seed_ranges", "cdc_seed_scan", "cdc_scan_get_stats", "cdc_best_track",
-           "cdc_find_tracks_host", "cdc_fp32_peak_probe"]
+           "cdc_find_tracks_host", "cdc_fp32_peak_probe", "cdc_kernel_launch_count"]
 
 
 class CdcError(RuntimeError):
@@ -55,7 +55,7 @@ class HoughParams(C.Structure):
 
 class ScanStats(C.Structure):
     _fields_ = [(k, C.c_uint64) for k in ("n_seeds", "n_steps", "n_gas_steps", "n_approach_tests", "n_pool",
-                                          "pool_cap")]
+                                          "pool_cap", "n_lookups", "n_g1", "n_approaches")] + [("kernel_ms", C.c_double)]
 
 
 SEED_DEBUG_DTYPE = np.dtype([("n_steps", "i4"), ("turns", "i4"), ("m_gas", "i4"), ("pad", "i4"),
@@ -77,6 +77,7 @@ def lib():
         L.cdc_last_error.restype = C.c_char_p
         for name in EXPORTS[1:]:
             getattr(L, name).restype = C.c_int32
+        L.cdc_kernel_launch_count.restype = C.c_uint64
         _lib = L
     return _lib
 
@@ -222,7 +223,7 @@ def cdc_seed_scan(geometry: Geometry, events: Events, grids: C.Array, params: Sc
 def cdc_scan_get_stats(events: Events, stream=None) -> dict:
     st = ScanStats()
     _check(lib().cdc_scan_get_stats(events.handle, C.byref(st), _stream(stream)))
-    return {k: int(getattr(st, k)) for k, _ in ScanStats._fields_}
+    return {k: (float if k == "kernel_ms" else int)(getattr(st, k)) for k, _ in ScanStats._fields_}
 
 
 def cdc_best_track(geometry: Geometry, events: Events, grids: C.Array, params: ScanParams, d_best_key, d_best_seed,
@@ -247,6 +248,10 @@ def cdc_find_tracks_host(geometry: Geometry, hit_offsets, wire_id, drift_mm, gri
                                       _hp(key), _hp(lab), _hp(ranges), _stream(stream)))
     return dict(best_seed=seed, best_n_match=nm, best_chi2=chi2, best_key=key, labels=lab[:int(off[-1])],
                 ranges=ranges)
+
+
+def cdc_kernel_launch_count() -> int:
+    return int(lib().cdc_kernel_launch_count())
 
 
 def cdc_fp32_peak_probe(iters: int = 4096, stream=None):

@@ -4,6 +4,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <atomic>
 #include <new>
 
 #include "cdc_internal.cuh"
@@ -12,6 +13,10 @@ static thread_local std::string g_last_error;
 void cdc_set_error(const std::string &msg) { g_last_error = msg; }
 
 extern "C" const char *cdc_last_error(void) { return g_last_error.c_str(); }
+
+static std::atomic<uint64_t> g_launches{0};
+void cdc_count_launch(int n) { g_launches.fetch_add((uint64_t)n, std::memory_order_relaxed); }
+extern "C" uint64_t cdc_kernel_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 namespace {
 

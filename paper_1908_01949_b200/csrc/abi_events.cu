@@ -17,6 +17,10 @@ void free_events(cdc_events *ev)
     cudaFree(ev->d_counters); cudaFree(ev->d_pool_S64); cudaFree(ev->d_pool_chi2); cudaFree(ev->d_pool_nmatch);
     cudaFree(ev->d_ev_maxS); cudaFree(ev->d_ev_best); cudaFree(ev->d_wire_label); cudaFree(ev->d_wire_best);
     cudaFree(ev->d_peak_key);
+    cudaFreeHost(ev->h_axes_pinned); cudaFreeHost(ev->h_grids_pinned);
+    if (ev->ev_k0) cudaEventDestroy(ev->ev_k0);
+    if (ev->ev_k1) cudaEventDestroy(ev->ev_k1);
+    if (ev->ev_copy) cudaEventDestroy(ev->ev_copy);
     delete ev;
 }
 

@@ -51,9 +51,20 @@ int32_t prepare_grids(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec
         ev->axes.stride = stride;
     }
     stride = ev->axes.stride;
-    std::vector<double> tab((size_t)E * 6 * stride, 0.0);
+    const size_t n_tab = (size_t)E * 6 * stride;
+    // pinned staging owned by the handle: the copies are truly asynchronous; wait only if the previous
+    // scan's copy of the same staging buffer has not finished yet
+    if (!ev->ev_copy) CDC_CUDA(cudaEventCreateWithFlags(&ev->ev_copy, cudaEventDisableTiming));
+    else CDC_CUDA(cudaEventSynchronize(ev->ev_copy));
+    if (ev->h_axes_cap < n_tab) {
+        cudaFreeHost(ev->h_axes_pinned); ev->h_axes_pinned = nullptr; ev->h_axes_cap = 0;
+        CDC_CUDA(cudaMallocHost((void **)&ev->h_axes_pinned, sizeof(double) * n_tab));
+        ev->h_axes_cap = n_tab;
+    }
+    if (!ev->h_grids_pinned) CDC_CUDA(cudaMallocHost((void **)&ev->h_grids_pinned, sizeof(GridDev) * (size_t)E));
+    double *tab = ev->h_axes_pinned;
     for (int e = 0; e < E; ++e) {
-        double *t = tab.data() + (size_t)e * 6 * stride;
+        double *t = tab + (size_t)e * 6 * stride;
         const cdc_grid_spec &G = grids[e];
         for (int i = 0; i < G.n[0]; ++i) {            // reading C4: r0 = (R0 cos(theta), R0 sin(theta), z)
             const double th = G.lo[0] + (double)i * G.step[0];
@@ -62,10 +73,11 @@ int32_t prepare_grids(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec
         }
         for (int a = 1; a < 5; ++a)
             for (int i = 0; i < G.n[a]; ++i) t[(size_t)(a + 1) * stride + i] = G.lo[a] + (double)i * G.step[a];
+        ev->h_grids_pinned[e] = ev->h_grids[e];
     }
-    CDC_CUDA(cudaMemcpyAsync(ev->axes.d, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice, s));
-    CDC_CUDA(cudaMemcpyAsync(ev->d_grids, ev->h_grids.data(), sizeof(GridDev) * (size_t)E, cudaMemcpyHostToDevice, s));
-    CDC_CUDA(cudaStreamSynchronize(s));               // `tab` is pageable and about to go out of scope
+    CDC_CUDA(cudaMemcpyAsync(ev->axes.d, tab, sizeof(double) * n_tab, cudaMemcpyHostToDevice, s));
+    CDC_CUDA(cudaMemcpyAsync(ev->d_grids, ev->h_grids_pinned, sizeof(GridDev) * (size_t)E, cudaMemcpyHostToDevice, s));
+    CDC_CUDA(cudaEventRecord(ev->ev_copy, s));
     return CDC_OK;
 }
 
@@ -144,7 +156,8 @@ extern "C" int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cd
     L.d_pool = ev->d_pool; L.pool_cap = ev->pool_cap; L.d_counters = ev->d_counters;
     L.max_seeds_per_event = 0;
     for (const GridDev &G : ev->h_grids) L.max_seeds_per_event = std::max<int64_t>(L.max_seeds_per_event, G.n_seeds);
-    CDC_CUDA(launch_seed_scan(L, s));
+    if (!ev->ev_k0) { CDC_CUDA(cudaEventCreate(&ev->ev_k0)); CDC_CUDA(cudaEventCreate(&ev->ev_k1)); }
+    CDC_CUDA(launch_seed_scan(L, s, ev->ev_k0, ev->ev_k1));
     ev->scanned = true;
     return CDC_OK;
 }
@@ -160,6 +173,11 @@ extern "C" int32_t cdc_scan_get_stats(const cdc_events *ev, cdc_scan_stats *out,
     for (const GridDev &G : ev->h_grids) out->n_seeds += (uint64_t)G.n_seeds;
     out->n_steps = c[CNT_STEPS]; out->n_gas_steps = c[CNT_GAS]; out->n_approach_tests = c[CNT_TESTS];
     out->n_pool = c[CNT_POOL]; out->pool_cap = ev->pool_cap;
+    out->n_lookups = c[CNT_LOOKUP]; out->n_g1 = c[CNT_G1]; out->n_approaches = c[CNT_APPROACH];
+    float ms = 0.f;
+    CDC_CUDA(cudaEventSynchronize(ev->ev_k1));
+    CDC_CUDA(cudaEventElapsedTime(&ms, ev->ev_k0, ev->ev_k1));
+    out->kernel_ms = (double)ms;
     return CDC_OK;
 }
 

@@ -291,7 +291,9 @@ cudaError_t launch_best_track(const BestLaunch &L, cudaStream_t s)
     fill_i32<<<(unsigned)((nw + 255) / 256), 256, 0, s>>>(L.d_wire_label, nw, -1);
     label_kernel<<<(L.n_events + 31) / 32, 32, 0, s>>>(A, L.n_events, L.d_ev_best, L.d_wire_label, L.d_wire_best,
                                                          L.d_best_seed, L.d_best_n_match, L.d_best_chi2);
+    cdc_count_launch(4);
     if (L.max_hits_per_event > 0 && L.d_labels) {
+        cdc_count_launch();
         dim3 grid((unsigned)((L.max_hits_per_event + 127) / 128), (unsigned)L.n_events);
         gather_labels<<<grid, 128, 0, s>>>(L.W, L.d_offsets, L.d_wire_id, L.d_wire_label, L.d_labels);
     }

@@ -110,6 +110,10 @@ struct cdc_events {
     uint32_t pool_cap = 0;
     unsigned long long *d_counters = nullptr;   // [8]: steps, gas steps, approach tests, pool count, ...
     bool scanned = false;
+    cudaEvent_t ev_k0 = nullptr, ev_k1 = nullptr, ev_copy = nullptr;   // scan kernel bracket; axis-table copy done
+    double *h_axes_pinned = nullptr;
+    size_t h_axes_cap = 0;
+    GridDev *h_grids_pinned = nullptr;
     // best-track scratch
     double *d_pool_S64 = nullptr, *d_pool_chi2 = nullptr;
     int32_t *d_pool_nmatch = nullptr;
@@ -121,7 +125,9 @@ struct cdc_events {
     int32_t max_hits_per_event = 0;
 };
 
-enum { CNT_STEPS = 0, CNT_GAS = 1, CNT_TESTS = 2, CNT_POOL = 3, CNT_N = 8 };
+enum { CNT_STEPS = 0, CNT_GAS = 1, CNT_TESTS = 2, CNT_POOL = 3, CNT_LOOKUP = 4, CNT_G1 = 5, CNT_APPROACH = 6, CNT_N = 8 };
+
+void cdc_count_launch(int n = 1);
 
 // ---- error plumbing ------------------------------------------------------------------------------
 void cdc_set_error(const std::string &msg);
@@ -153,7 +159,7 @@ struct ScanLaunch {
     unsigned long long *d_counters;
     int64_t max_seeds_per_event;
 };
-cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s);
+cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0, cudaEvent_t k1);
 
 cudaError_t launch_bin_events(int32_t n_events, int32_t W, int32_t n_bit_words, int32_t max_hits_per_event,
                               const int32_t *d_offsets, const int32_t *d_wire_id, const float *d_drift,

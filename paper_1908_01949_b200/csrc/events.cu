@@ -40,9 +40,11 @@ cudaError_t launch_bin_events(int32_t n_events, int32_t W, int32_t n_bit_words, 
     e = cudaMemsetAsync(d_err, 0, sizeof(int32_t), s);
     if (e != cudaSuccess) return e;
     fill_f32<<<(unsigned)((n_tab + 255) / 256), 256, 0, s>>>(d_drift_tab, n_tab, -1.0f);
+    cdc_count_launch();
     if (max_hits_per_event > 0) {
         dim3 grid((unsigned)((max_hits_per_event + 127) / 128), (unsigned)n_events);
         bin_hits<<<grid, 128, 0, s>>>(W, n_bit_words, d_offsets, d_wire_id, d_drift, d_drift_tab, d_bits, d_err);
+        cdc_count_launch();
     }
     return cudaGetLastError();
 }

@@ -151,6 +151,7 @@ cudaError_t launch_hough(const HoughLaunch &L, cudaStream_t s)
     }
     dim3 grid((unsigned)((L.ncy * L.ncx + kHBlock - 1) / kHBlock), (unsigned)L.n_events);
     hough_vote_kernel<<<grid, kHBlock, smem, s>>>(A);
+    cdc_count_launch(2);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     hough_finalize_kernel<<<(L.n_events + 63) / 64, 64, 0, s>>>(L.n_events, L.nR, L.ncy, L.ncx, L.bin_xy64, L.bin_R64,

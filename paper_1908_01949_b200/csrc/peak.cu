@@ -38,6 +38,7 @@ cudaError_t run_fp32_peak_probe(int32_t iters, double *flops_per_s, double *ms_o
     cudaEventRecord(t0, s);
     ffma_chain_kernel<<<blocks, 1024, 0, s>>>(iters, 1.0f, sink);
     cudaEventRecord(t1, s);
+    cdc_count_launch(2);
     e = cudaEventSynchronize(t1);
     float ms = 0.f;
     if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, t0, t1);

@@ -98,7 +98,7 @@ struct Vertex {            // what scoring needs of a step vertex
 
 // One candidate wire that has a hit: does interval n own an approach to it, and does the hit match?
 __device__ __forceinline__ void score_wire(const ScanArgs &A, const float *drift_e, int w, float uz, float inv_uz, const Vertex &v0,
-                                           const Vertex &v1, uint32_t &nm, float &chi2)
+                                           const Vertex &v1, uint32_t &nm, float &chi2, uint32_t &cnt)
 {
     float4 wr = __ldg(A.gd.wire4 + w);
     float zt0 = v0.z * inv_uz;
@@ -108,6 +108,7 @@ __device__ __forceinline__ void score_wire(const ScanArgs &A, const float *drift
     float eu0 = fmaf(ex0, wr.z, ey0 * wr.w);
     float g0 = fmaf(ex0, v0.Tx, fmaf(ey0, v0.Ty, -eu0 * uT0));   // g = delta . T, delta = e - (e.u) u
     if (!(g0 <= 0.0f)) return;
+    cnt += 1u;                                                // packed: g1 evaluations | owned approaches << 16
     float zt1 = v1.z * inv_uz;
     float ex1 = fmaf(-zt1, wr.z, v1.x - wr.x) + v1.xl;
     float ey1 = fmaf(-zt1, wr.w, v1.y - wr.y) + v1.yl;
@@ -115,6 +116,7 @@ __device__ __forceinline__ void score_wire(const ScanArgs &A, const float *drift
     float eu1 = fmaf(ex1, wr.z, ey1 * wr.w);
     float g1 = fmaf(ex1, v1.Tx, fmaf(ey1, v1.Ty, -eu1 * uT1));
     if (!(g1 > 0.0f)) return;
+    cnt += 1u << 16;
     float tau = __fdividef(g0, g0 - g1);
     float ex = fmaf(tau, ex1 - ex0, ex0);                   // e is linear in the position: exact chord point
     float ey = fmaf(tau, ey1 - ey0, ey0);
@@ -130,7 +132,7 @@ __device__ __forceinline__ void score_wire(const ScanArgs &A, const float *drift
 
 __device__ __forceinline__ void score_layer(const ScanArgs &A, const float *drift_e, const LayerDev *s_layer, const uint32_t *s_bits,
                                             int j, float phi, const Vertex &v0, const Vertex &v1, uint32_t &nm,
-                                            float &chi2, uint32_t &tests)
+                                            float &chi2, uint32_t &tests, uint32_t &cnt)
 {
     if ((unsigned)j >= (unsigned)A.gd.n_layers) return;
     const LayerDev L = s_layer[j];
@@ -143,8 +145,8 @@ __device__ __forceinline__ void score_layer(const ScanArgs &A, const float *drif
     k1 += (k1 < 0) ? L.n : 0; k1 += (k1 < 0) ? L.n : 0; k1 -= (k1 >= L.n) ? L.n : 0;
     k2 += (k2 < 0) ? L.n : 0; k2 += (k2 < 0) ? L.n : 0; k2 -= (k2 >= L.n) ? L.n : 0;
     int w1 = L.offset + k1, w2 = L.offset + k2;
-    if ((s_bits[w1 >> 5] >> (w1 & 31)) & 1u) { tests += 1u; score_wire(A, drift_e, w1, L.uz, L.inv_uz, v0, v1, nm, chi2); }
-    if ((s_bits[w2 >> 5] >> (w2 & 31)) & 1u) { tests += 1u; score_wire(A, drift_e, w2, L.uz, L.inv_uz, v0, v1, nm, chi2); }
+    if ((s_bits[w1 >> 5] >> (w1 & 31)) & 1u) { tests += 1u; score_wire(A, drift_e, w1, L.uz, L.inv_uz, v0, v1, nm, chi2, cnt); }
+    if ((s_bits[w2 >> 5] >> (w2 & 31)) & 1u) { tests += 1u; score_wire(A, drift_e, w2, L.uz, L.inv_uz, v0, v1, nm, chi2, cnt); }
 }
 
 __device__ __forceinline__ unsigned long long warp_max_u64(unsigned long long v)
@@ -205,7 +207,7 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
     }
     const bool low_p = !(p0h > 1.0f);                 // p <= 1 MeV/c ends a track after its first step (C7)
 
-    uint32_t nm = 0, tests = 0;
+    uint32_t nm = 0, tests = 0, cnt = 0, lookups = 0;
     float chi2 = 0.0f;
     int n = 0, m = 0, turn = 0;
     bool cn = true;                                   // c_0 := true (reading C7)
@@ -258,14 +260,15 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
             if (u2 > A.gd.u2_lo && u2 < A.gd.u2_hi) {
                 Vertex v1;
                 v1.x = xh; v1.y = yh; v1.z = zh; v1.xl = xl; v1.yl = yl; v1.Tx = Txh; v1.Ty = Tyh; v1.Tz = Tzh;
+                lookups += 1u;
                 float u = u2 * rsqrtf(u2);
                 float fj = (u - A.gd.r_first) * A.gd.inv_pitch;
                 float jn = rintf(fj);
                 int jc = (int)jn;
                 int j2 = jc + ((fj - jn) >= 0.0f ? 1 : -1);
                 float phi = coarse_atan2(v0.y, v0.x);
-                score_layer(A, drift_e, s_layer, s_bits, jc, phi, v0, v1, nm, chi2, tests);
-                score_layer(A, drift_e, s_layer, s_bits, j2, phi, v0, v1, nm, chi2, tests);
+                score_layer(A, drift_e, s_layer, s_bits, jc, phi, v0, v1, nm, chi2, tests, cnt);
+                score_layer(A, drift_e, s_layer, s_bits, j2, phi, v0, v1, nm, chi2, tests, cnt);
             }
             m += 1;
         }
@@ -327,16 +330,22 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
     unsigned sn = __reduce_add_sync(0xffffffffu, valid ? (unsigned)n : 0u);
     unsigned sm = __reduce_add_sync(0xffffffffu, valid ? (unsigned)m : 0u);
     unsigned st = __reduce_add_sync(0xffffffffu, tests);
+    unsigned sl = __reduce_add_sync(0xffffffffu, lookups);
+    unsigned sg = __reduce_add_sync(0xffffffffu, cnt & 0xFFFFu);
+    unsigned sa = __reduce_add_sync(0xffffffffu, cnt >> 16);
     if (lane == 0) {
         atomicAdd(A.counters + CNT_STEPS, (unsigned long long)sn);
         atomicAdd(A.counters + CNT_GAS, (unsigned long long)sm);
         atomicAdd(A.counters + CNT_TESTS, (unsigned long long)st);
+        atomicAdd(A.counters + CNT_LOOKUP, (unsigned long long)sl);
+        atomicAdd(A.counters + CNT_G1, (unsigned long long)sg);
+        atomicAdd(A.counters + CNT_APPROACH, (unsigned long long)sa);
     }
 }
 
 }  // namespace
 
-cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s)
+cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0, cudaEvent_t k1)
 {
     ScanArgs A;
     A.gd = L.gd; A.fd = L.fd; A.grids = L.d_grids; A.axes = L.d_axes; A.axis_stride = L.axis_stride;
@@ -353,6 +362,7 @@ cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s)
     if (L.gd.n_bit_words > kMaxBitWords || L.gd.n_layers > CDC_MAX_LAYERS) return cudaErrorInvalidValue;
     dim3 grid((unsigned)((L.max_seeds_per_event + kBlock - 1) / kBlock), (unsigned)L.n_events);
     const bool eloss = L.eloss_h != 0.0f;
+    if (k0) cudaEventRecord(k0, s);
     if (L.fd.kind == 0) {
         if (eloss) seed_scan_kernel<0, true><<<grid, kBlock, 0, s>>>(A);
         else seed_scan_kernel<0, false><<<grid, kBlock, 0, s>>>(A);
@@ -360,5 +370,7 @@ cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s)
         if (eloss) seed_scan_kernel<1, true><<<grid, kBlock, 0, s>>>(A);
         else seed_scan_kernel<1, false><<<grid, kBlock, 0, s>>>(A);
     }
+    if (k1) cudaEventRecord(k1, s);
+    cdc_count_launch();
     return cudaGetLastError();
 }
