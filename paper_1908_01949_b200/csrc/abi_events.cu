@@ -12,16 +12,36 @@ namespace {
 void free_events(cdc_events *ev)
 {
     if (!ev) return;
-    cudaFree(ev->d_offsets); cudaFree(ev->d_wire_id); cudaFree(ev->d_drift); cudaFree(ev->d_drift_tab);
-    cudaFree(ev->d_bits); cudaFree(ev->d_err); cudaFree(ev->axes.d); cudaFree(ev->d_grids); cudaFree(ev->d_pool);
-    cudaFree(ev->d_counters); cudaFree(ev->d_pool_S64); cudaFree(ev->d_pool_chi2); cudaFree(ev->d_pool_nmatch);
-    cudaFree(ev->d_ev_maxS); cudaFree(ev->d_ev_best); cudaFree(ev->d_wire_label); cudaFree(ev->d_wire_best);
-    cudaFree(ev->d_peak_key);
-    cudaFreeHost(ev->h_axes_pinned); cudaFreeHost(ev->h_grids_pinned);
+    // stream-ordered: the memory returns to the pool after the work already queued on the upload stream
+    if (ev->slab) cudaFreeAsync(ev->slab, ev->alloc_stream);
+    if (ev->axes.d) cudaFreeAsync(ev->axes.d, ev->alloc_stream);
     if (ev->ev_k0) cudaEventDestroy(ev->ev_k0);
     if (ev->ev_k1) cudaEventDestroy(ev->ev_k1);
-    if (ev->ev_copy) cudaEventDestroy(ev->ev_copy);
     delete ev;
+}
+
+struct Carver {                 // pass 1 (base == nullptr) sizes the slab, pass 2 hands out the pieces
+    char *base = nullptr;
+    size_t off = 0;
+    template <typename T>
+    void take(T *&p, size_t n)
+    {
+        const size_t bytes = (std::max<size_t>(n, 1) * sizeof(T) + 255) & ~(size_t)255;
+        if (base) p = reinterpret_cast<T *>(base + off);
+        off += bytes;
+    }
+};
+
+void carve(cdc_events *ev, Carver &c)
+{
+    const size_t E = (size_t)ev->n_events, W = (size_t)ev->W, H = (size_t)ev->total_hits, P = ev->pool_cap;
+    c.take(ev->d_offsets, E + 1); c.take(ev->d_wire_id, H); c.take(ev->d_drift, H);
+    c.take(ev->d_drift_tab, E * W); c.take(ev->d_bits, E * ev->n_bit_words); c.take(ev->d_err, 1);
+    c.take(ev->d_counters, CNT_N); c.take(ev->d_ev_maxS, E); c.take(ev->d_ev_best, E); c.take(ev->d_peak_key, E);
+    c.take(ev->d_wire_label, E * W); c.take(ev->d_wire_best, E * W); c.take(ev->d_grids, E);
+    c.take(ev->d_pool, P); c.take(ev->d_pool_S64, P); c.take(ev->d_pool_chi2, P); c.take(ev->d_pool_nmatch, P);
+    c.take(ev->d_pool_slot, P); c.take(ev->d_rec, (size_t)kRecSlots * kRecCap); c.take(ev->d_rec_count, kRecSlots);
+    c.take(ev->d_slot_counter, 1); c.take(ev->d_ev_slot, E);
 }
 
 }  // namespace
@@ -52,20 +72,14 @@ extern "C" int32_t cdc_event_upload(const cdc_geometry *g, int32_t n_events, con
     ev->geom = g; ev->n_events = n_events; ev->total_hits = total; ev->W = g->W; ev->n_bit_words = (g->W + 31) / 32;
     ev->max_hits_per_event = max_hits;
     ev->offsets.assign(h_hit_offsets, h_hit_offsets + n_events + 1);
-    const size_t nt = std::max<size_t>((size_t)total, 1);
-    EV_CUDA(cudaMalloc((void **)&ev->d_offsets, sizeof(int32_t) * (size_t)(n_events + 1)));
-    EV_CUDA(cudaMalloc((void **)&ev->d_wire_id, sizeof(int32_t) * nt));
-    EV_CUDA(cudaMalloc((void **)&ev->d_drift, sizeof(float) * nt));
-    EV_CUDA(cudaMalloc((void **)&ev->d_drift_tab, sizeof(float) * (size_t)n_events * g->W));
-    EV_CUDA(cudaMalloc((void **)&ev->d_bits, sizeof(uint32_t) * (size_t)n_events * ev->n_bit_words));
-    EV_CUDA(cudaMalloc((void **)&ev->d_err, sizeof(int32_t)));
-    EV_CUDA(cudaMalloc((void **)&ev->d_counters, sizeof(unsigned long long) * CNT_N));
-    EV_CUDA(cudaMalloc((void **)&ev->d_ev_maxS, sizeof(unsigned long long) * (size_t)n_events));
-    EV_CUDA(cudaMalloc((void **)&ev->d_ev_best, sizeof(unsigned long long) * (size_t)n_events));
-    EV_CUDA(cudaMalloc((void **)&ev->d_peak_key, sizeof(unsigned long long) * (size_t)n_events));
-    EV_CUDA(cudaMalloc((void **)&ev->d_wire_label, sizeof(int32_t) * (size_t)n_events * g->W));
-    EV_CUDA(cudaMalloc((void **)&ev->d_wire_best, sizeof(double) * (size_t)n_events * g->W));
-    EV_CUDA(cudaMalloc((void **)&ev->d_grids, sizeof(GridDev) * (size_t)n_events));
+    ev->pool_cap = std::max<uint32_t>(1u << 16, 64u * (uint32_t)n_events);
+    ev->alloc_stream = s;
+    Carver sizing;
+    carve(ev, sizing);
+    EV_CUDA(cudaMallocAsync(&ev->slab, sizing.off, s));
+    Carver placing;
+    placing.base = static_cast<char *>(ev->slab);
+    carve(ev, placing);
     EV_CUDA(cudaMemsetAsync(ev->d_counters, 0, sizeof(unsigned long long) * CNT_N, s));
     EV_CUDA(cudaMemcpyAsync(ev->d_offsets, h_hit_offsets, sizeof(int32_t) * (size_t)(n_events + 1), cudaMemcpyHostToDevice, s));
     if (total > 0) {

@@ -3,13 +3,43 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 
 #include "cdc_internal.cuh"
 
 namespace {
 
-constexpr uint32_t kPoolCap = 1u << 20;
 constexpr double kDefaultMargin = 0.05;
+
+// One pinned host buffer per process for the small per-scan tables (axis nodes, grid records).  acquire() waits
+// for the previous copy out of it (an event), so consecutive scans on any stream never overwrite live data.
+struct Staging {
+    std::mutex mu;
+    char *p = nullptr;
+    size_t cap = 0;
+    cudaEvent_t done = nullptr;
+    int32_t acquire(size_t bytes, char **out)
+    {
+        mu.lock();
+        if (!done) { cudaError_t e = cudaEventCreateWithFlags(&done, cudaEventDisableTiming); if (e != cudaSuccess) { mu.unlock(); CDC_FAIL(CDC_ERR_CUDA, "staging event"); } }
+        else cudaEventSynchronize(done);
+        if (cap < bytes) {
+            if (p) cudaFreeHost(p);
+            p = nullptr; cap = 0;
+            const size_t want = std::max<size_t>(bytes, 1 << 16);
+            if (cudaMallocHost((void **)&p, want) != cudaSuccess) { mu.unlock(); CDC_FAIL(CDC_ERR_NOMEM, "pinned staging allocation failed"); }
+            cap = want;
+        }
+        *out = p;
+        return CDC_OK;       // still locked: release() unlocks
+    }
+    cudaError_t release(cudaStream_t s)
+    {
+        cudaError_t e = cudaEventRecord(done, s);
+        mu.unlock();
+        return e;
+    }
+} g_staging;
 
 int32_t check_params(const cdc_scan_params *p, const char *who)
 {
@@ -46,23 +76,23 @@ int32_t prepare_grids(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec
         off += prod;
     }
     if (ev->axes.stride < stride) {
-        cudaFree(ev->axes.d); ev->axes.d = nullptr; ev->axes.stride = 0;
-        CDC_CUDA(cudaMalloc((void **)&ev->axes.d, sizeof(double) * (size_t)E * 6 * stride));
+        if (ev->axes.d) CDC_CUDA(cudaFreeAsync(ev->axes.d, s));
+        ev->axes.d = nullptr; ev->axes.stride = 0;
+        CDC_CUDA(cudaMallocAsync((void **)&ev->axes.d, sizeof(double) * (size_t)E * 6 * stride, s));
         ev->axes.stride = stride;
     }
     stride = ev->axes.stride;
     const size_t n_tab = (size_t)E * 6 * stride;
-    // pinned staging owned by the handle: the copies are truly asynchronous; wait only if the previous
-    // scan's copy of the same staging buffer has not finished yet
-    if (!ev->ev_copy) CDC_CUDA(cudaEventCreateWithFlags(&ev->ev_copy, cudaEventDisableTiming));
-    else CDC_CUDA(cudaEventSynchronize(ev->ev_copy));
-    if (ev->h_axes_cap < n_tab) {
-        cudaFreeHost(ev->h_axes_pinned); ev->h_axes_pinned = nullptr; ev->h_axes_cap = 0;
-        CDC_CUDA(cudaMallocHost((void **)&ev->h_axes_pinned, sizeof(double) * n_tab));
-        ev->h_axes_cap = n_tab;
+    // process-wide pinned staging: the copies are truly asynchronous; wait only if the previous user's copy
+    // out of the staging buffer has not finished yet
+    const size_t grid_off = (sizeof(double) * n_tab + 255) & ~(size_t)255;
+    char *stage = nullptr;
+    {
+        const int32_t rc = g_staging.acquire(grid_off + sizeof(GridDev) * (size_t)E, &stage);
+        if (rc != CDC_OK) return rc;
     }
-    if (!ev->h_grids_pinned) CDC_CUDA(cudaMallocHost((void **)&ev->h_grids_pinned, sizeof(GridDev) * (size_t)E));
-    double *tab = ev->h_axes_pinned;
+    double *tab = reinterpret_cast<double *>(stage);
+    GridDev *h_grids_pinned = reinterpret_cast<GridDev *>(stage + grid_off);
     for (int e = 0; e < E; ++e) {
         double *t = tab + (size_t)e * 6 * stride;
         const cdc_grid_spec &G = grids[e];
@@ -73,23 +103,12 @@ int32_t prepare_grids(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec
         }
         for (int a = 1; a < 5; ++a)
             for (int i = 0; i < G.n[a]; ++i) t[(size_t)(a + 1) * stride + i] = G.lo[a] + (double)i * G.step[a];
-        ev->h_grids_pinned[e] = ev->h_grids[e];
+        h_grids_pinned[e] = ev->h_grids[e];
     }
-    CDC_CUDA(cudaMemcpyAsync(ev->axes.d, tab, sizeof(double) * n_tab, cudaMemcpyHostToDevice, s));
-    CDC_CUDA(cudaMemcpyAsync(ev->d_grids, ev->h_grids_pinned, sizeof(GridDev) * (size_t)E, cudaMemcpyHostToDevice, s));
-    CDC_CUDA(cudaEventRecord(ev->ev_copy, s));
-    return CDC_OK;
-}
-
-int32_t ensure_pool(cdc_events *ev)
-{
-    if (ev->d_pool) return CDC_OK;
-    const uint32_t cap = std::max<uint32_t>(kPoolCap, 256u * (uint32_t)ev->n_events);
-    CDC_CUDA(cudaMalloc((void **)&ev->d_pool, sizeof(PoolEntry) * (size_t)cap));
-    CDC_CUDA(cudaMalloc((void **)&ev->d_pool_S64, sizeof(double) * (size_t)cap));
-    CDC_CUDA(cudaMalloc((void **)&ev->d_pool_chi2, sizeof(double) * (size_t)cap));
-    CDC_CUDA(cudaMalloc((void **)&ev->d_pool_nmatch, sizeof(int32_t) * (size_t)cap));
-    ev->pool_cap = cap;
+    const cudaError_t c1 = cudaMemcpyAsync(ev->axes.d, tab, sizeof(double) * n_tab, cudaMemcpyHostToDevice, s);
+    const cudaError_t c2 = cudaMemcpyAsync(ev->d_grids, h_grids_pinned, sizeof(GridDev) * (size_t)E, cudaMemcpyHostToDevice, s);
+    const cudaError_t c3 = g_staging.release(s);          // always unlocks
+    CDC_CUDA(c1); CDC_CUDA(c2); CDC_CUDA(c3);
     return CDC_OK;
 }
 
@@ -142,7 +161,6 @@ extern "C" int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cd
     if (rc != CDC_OK) return rc;
     cudaStream_t s = (cudaStream_t)stream;
     if ((rc = prepare_grids(g, ev, h_grids, s)) != CDC_OK) return rc;
-    if ((rc = ensure_pool(ev)) != CDC_OK) return rc;
     CDC_CUDA(cudaMemsetAsync(d_best_key, 0, sizeof(uint64_t) * (size_t)ev->n_events, s));
     CDC_CUDA(cudaMemsetAsync(ev->d_counters, 0, sizeof(unsigned long long) * CNT_N, s));
     ScanLaunch L;
@@ -204,6 +222,8 @@ extern "C" int32_t cdc_best_track(const cdc_geometry *g, cdc_events *ev, const c
     L.d_best_key = d_best_key; L.d_pool = ev->d_pool; L.pool_cap = ev->pool_cap; L.d_counters = ev->d_counters;
     L.d_pool_S64 = ev->d_pool_S64; L.d_pool_chi2 = ev->d_pool_chi2; L.d_pool_nmatch = ev->d_pool_nmatch;
     L.d_ev_maxS = ev->d_ev_maxS; L.d_ev_best = ev->d_ev_best; L.d_wire_label = ev->d_wire_label; L.d_wire_best = ev->d_wire_best;
+    L.d_rec = ev->d_rec; L.d_rec_count = ev->d_rec_count; L.d_pool_slot = ev->d_pool_slot; L.d_slot_counter = ev->d_slot_counter;
+    L.d_ev_slot = ev->d_ev_slot;
     L.d_best_seed = d_best_seed; L.d_best_n_match = d_best_n_match; L.d_best_chi2 = d_best_chi2; L.d_labels = d_labels;
     CDC_CUDA(launch_best_track(L, (cudaStream_t)stream));
     return CDC_OK;

@@ -109,8 +109,8 @@ __device__ int candidates64(const Geom64 &g, const uint32_t *bits, const double 
         const float kf = (phi - L.phi0 - atanf(z * L.shift_k)) * L.kscale;
         const int kc = (int)rintf(kf);
         for (int dk = -1; dk <= 1; ++dk) {
-            int k = (kc + dk) % L.n;
-            if (k < 0) k += L.n;
+            int k = kc + dk;                                         // |k| < 2 n: wrap without a division
+            k += (k < 0) ? L.n : 0; k += (k < 0) ? L.n : 0; k -= (k >= L.n) ? L.n : 0;
             const int w = L.offset + k;
             if (!((bits[w >> 5] >> (w & 31)) & 1u)) continue;
             int i = n++;
@@ -128,7 +128,7 @@ struct Eval64 {
 
 // readings C4-C10: evaluate one seed.  wire_label / wire_best (optional, per wire of this event): reading C12.
 __device__ void eval_seed64(const BestArgs &A, int e, uint32_t index, Eval64 &out, int32_t *wire_label,
-                            double *wire_best)
+                            double *wire_best, ApproachRec *rec, int32_t *rec_count)
 {
     const GridDev G = A.grids[e];
     uint32_t q = index;
@@ -145,11 +145,12 @@ __device__ void eval_seed64(const BestArgs &A, int e, uint32_t index, Eval64 &ou
     double p = p0, chi2 = 0.0;
     const uint32_t *bits = A.bits + (size_t)e * A.n_bit_words;
     const float *drift = A.drift_tab + (size_t)e * A.W;
-    int n = 0, turn = 0, m = 0, n_match = 0;
+    int n = 0, turn = 0, m = 0, n_match = 0, n_rec = 0;
     bool cn = true;
     int cand[9];
+    double a = A.kq / p, p_of_a = p;
     while (n < A.max_steps) {
-        const double a = A.kq / p;
+        if (p != p_of_a) { a = A.kq / p; p_of_a = p; }                  // a = kappa q / p_n (C5/C6)
         double rn[3], Tn[3];
         rkn_step64(A.g, a, A.h, r, T, rn, Tn);
         if (cn) {
@@ -175,6 +176,10 @@ __device__ void eval_seed64(const BestArgs &A, int e, uint32_t index, Eval64 &ou
                 if (fabs(zw) <= A.g.z_half && resid * resid < A.lambda) {
                     n_match += 1;
                     chi2 += resid * resid;
+                    if (rec) {                      // matched approaches in path order, replayed by label_kernel
+                        if (n_rec < kRecCap) { rec[n_rec].wire = w; rec[n_rec].turn = turn; rec[n_rec].absd = fabs(resid); }
+                        n_rec += 1;
+                    }
                     if (wire_label) {               // C12: smallest |resid| wins, ties -> earliest
                         const double ad = fabs(resid);
                         if (wire_label[w] < 0 || ad < wire_best[w]) { wire_label[w] = turn; wire_best[w] = ad; }
@@ -197,6 +202,7 @@ __device__ void eval_seed64(const BestArgs &A, int e, uint32_t index, Eval64 &ou
             break;
     }
     out.n_match = n_match; out.chi2 = chi2; out.n_steps = n; out.turns = turn; out.m_gas = m;
+    if (rec_count) *rec_count = n_rec;
 }
 
 __device__ __forceinline__ uint32_t pool_size(const unsigned long long *counters, uint32_t cap)
@@ -215,14 +221,19 @@ __device__ __forceinline__ bool qualifies(const PoolEntry &pe, const uint64_t *b
 __global__ void rescore_kernel(const BestArgs A, const PoolEntry *pool, uint32_t pool_cap,
                                const unsigned long long *counters, const uint64_t *best_key, float margin,
                                double *pool_S64, double *pool_chi2, int32_t *pool_nmatch,
-                               unsigned long long *ev_maxS)
+                               unsigned long long *ev_maxS, ApproachRec *rec, int32_t *rec_count, int32_t *pool_slot,
+                               int32_t *slot_counter)
 {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= pool_size(counters, pool_cap)) return;
     const PoolEntry pe = pool[i];
-    if (!qualifies(pe, best_key, margin)) { pool_S64[i] = -1.0; return; }
+    if (!qualifies(pe, best_key, margin)) { pool_S64[i] = -1.0; pool_slot[i] = -1; return; }
     Eval64 ev;
-    eval_seed64(A, (int)pe.event, pe.index, ev, nullptr, nullptr);
+    const int slot = atomicAdd(slot_counter, 1);
+    const bool have = slot < kRecSlots;
+    pool_slot[i] = have ? slot : -1;
+    eval_seed64(A, (int)pe.event, pe.index, ev, nullptr, nullptr, have ? rec + (size_t)slot * kRecCap : nullptr,
+                have ? rec_count + slot : nullptr);
     const double S = (double)ev.n_match - ev.chi2 / A.lambda;           // C10
     pool_S64[i] = S; pool_chi2[i] = ev.chi2; pool_nmatch[i] = ev.n_match;
     atomicMax(ev_maxS + pe.event, (unsigned long long)__double_as_longlong(S > 0.0 ? S : 0.0));
@@ -240,9 +251,26 @@ __global__ void pick_kernel(const PoolEntry *pool, uint32_t pool_cap, const unsi
     if ((unsigned long long)__double_as_longlong(S) == ev_maxS[pe.event]) atomicMin(ev_best + pe.event, (unsigned long long)pe.index);
 }
 
+// the record slot of each event's best seed (several pool entries may carry the same seed: any of them serves)
+__global__ void slot_kernel(const PoolEntry *pool, uint32_t pool_cap, const unsigned long long *counters,
+                            const double *pool_S64, const unsigned long long *ev_best, const int32_t *pool_slot,
+                            const int32_t *rec_count, int32_t *ev_slot)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= pool_size(counters, pool_cap)) return;
+    if (pool_S64[i] < 0.0) return;
+    const PoolEntry pe = pool[i];
+    const int slot = pool_slot[i];
+    if ((unsigned long long)pe.index == ev_best[pe.event] && slot >= 0 && rec_count[slot] <= kRecCap)
+        atomicMax(ev_slot + pe.event, slot);
+}
+
 // one thread per event: re-propagate the best seed, label wires, report (index, n_match, chi2)
 __global__ void label_kernel(const BestArgs A, int n_events, const unsigned long long *ev_best, int32_t *wire_label,
-                             double *wire_best, int64_t *best_seed, uint32_t *best_n_match, double *best_chi2)
+                             double *wire_best, int64_t *best_seed, uint32_t *best_n_match, double *best_chi2,
+                             const PoolEntry *pool, uint32_t pool_cap, const unsigned long long *counters,
+                             const double *pool_chi2, const int32_t *pool_nmatch, const int32_t *pool_slot,
+                             const ApproachRec *rec, const int32_t *rec_count, const int32_t *ev_slot)
 {
     const int e = blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= n_events) return;
@@ -251,8 +279,26 @@ __global__ void label_kernel(const BestArgs A, int n_events, const unsigned long
         best_seed[e] = -1; best_n_match[e] = 0; best_chi2[e] = 0.0;
         return;
     }
-    Eval64 ev;
-    eval_seed64(A, e, (uint32_t)b, ev, wire_label + (size_t)e * A.W, wire_best + (size_t)e * A.W);
+    const int slot = ev_slot[e];
+    if (slot >= 0) {                       // replay the recorded matched approaches (path order) -- reading C12
+        int32_t *lab = wire_label + (size_t)e * A.W;
+        double *bst = wire_best + (size_t)e * A.W;
+        const ApproachRec *r = rec + (size_t)slot * kRecCap;
+        const int n = rec_count[slot];
+        double chi2 = 0.0;
+        for (int i = 0; i < n; ++i) {
+            const int w = r[i].wire;
+            if (lab[w] < 0 || r[i].absd < bst[w]) { lab[w] = r[i].turn; bst[w] = r[i].absd; }
+        }
+        // n_match / chi2 of that pool entry
+        const uint32_t np = pool_size(counters, pool_cap);
+        for (uint32_t i = 0; i < np; ++i)
+            if (pool_slot[i] == slot) { chi2 = pool_chi2[i]; best_n_match[e] = (uint32_t)pool_nmatch[i]; break; }
+        best_seed[e] = (int64_t)b; best_chi2[e] = chi2;
+        return;
+    }
+    Eval64 ev;                             // no usable record (slot table full or list overflow): propagate again
+    eval_seed64(A, e, (uint32_t)b, ev, wire_label + (size_t)e * A.W, wire_best + (size_t)e * A.W, nullptr, nullptr);
     best_seed[e] = (int64_t)b; best_n_match[e] = (uint32_t)ev.n_match; best_chi2[e] = ev.chi2;
 }
 
@@ -283,15 +329,22 @@ cudaError_t launch_best_track(const BestLaunch &L, cudaStream_t s)
     cudaError_t e;
     if ((e = cudaMemsetAsync(L.d_ev_maxS, 0, sizeof(unsigned long long) * (size_t)L.n_events, s)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(L.d_ev_best, 0xFF, sizeof(unsigned long long) * (size_t)L.n_events, s)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(L.d_ev_slot, 0xFF, sizeof(int32_t) * (size_t)L.n_events, s)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(L.d_slot_counter, 0, sizeof(int32_t), s)) != cudaSuccess) return e;
     const unsigned nb = (L.pool_cap + 63) / 64;
     rescore_kernel<<<nb, 64, 0, s>>>(A, L.d_pool, L.pool_cap, L.d_counters, L.d_best_key, L.margin, L.d_pool_S64,
-                                     L.d_pool_chi2, L.d_pool_nmatch, L.d_ev_maxS);
+                                     L.d_pool_chi2, L.d_pool_nmatch, L.d_ev_maxS, L.d_rec, L.d_rec_count, L.d_pool_slot,
+                                     L.d_slot_counter);
     pick_kernel<<<nb, 64, 0, s>>>(L.d_pool, L.pool_cap, L.d_counters, L.d_pool_S64, L.d_ev_maxS, L.d_ev_best);
+    slot_kernel<<<nb, 64, 0, s>>>(L.d_pool, L.pool_cap, L.d_counters, L.d_pool_S64, L.d_ev_best, L.d_pool_slot,
+                                  L.d_rec_count, L.d_ev_slot);
     const size_t nw = (size_t)L.n_events * L.W;
     fill_i32<<<(unsigned)((nw + 255) / 256), 256, 0, s>>>(L.d_wire_label, nw, -1);
     label_kernel<<<(L.n_events + 31) / 32, 32, 0, s>>>(A, L.n_events, L.d_ev_best, L.d_wire_label, L.d_wire_best,
-                                                         L.d_best_seed, L.d_best_n_match, L.d_best_chi2);
-    cdc_count_launch(4);
+                                                         L.d_best_seed, L.d_best_n_match, L.d_best_chi2, L.d_pool,
+                                                         L.pool_cap, L.d_counters, L.d_pool_chi2, L.d_pool_nmatch,
+                                                         L.d_pool_slot, L.d_rec, L.d_rec_count, L.d_ev_slot);
+    cdc_count_launch(5);
     if (L.max_hits_per_event > 0 && L.d_labels) {
         cdc_count_launch();
         dim3 grid((unsigned)((L.max_hits_per_event + 127) / 128), (unsigned)L.n_events);

@@ -81,6 +81,13 @@ struct PoolEntry {           // one rescoring candidate (reading C11)
     uint32_t pad;
 };
 
+struct ApproachRec {         // one matched approach of a re-scored seed (reading C12)
+    int32_t wire, turn;
+    double absd;
+};
+constexpr int kRecSlots = 256;
+constexpr int kRecCap = 2048;
+
 struct AxisTables {          // per event, device: seed-axis node values in fp64 (A3)
     // layout [n_events][6][stride]: R0 cos(theta), R0 sin(theta), z, px, py, pz
     double *d = nullptr;
@@ -110,10 +117,7 @@ struct cdc_events {
     uint32_t pool_cap = 0;
     unsigned long long *d_counters = nullptr;   // [8]: steps, gas steps, approach tests, pool count, ...
     bool scanned = false;
-    cudaEvent_t ev_k0 = nullptr, ev_k1 = nullptr, ev_copy = nullptr;   // scan kernel bracket; axis-table copy done
-    double *h_axes_pinned = nullptr;
-    size_t h_axes_cap = 0;
-    GridDev *h_grids_pinned = nullptr;
+    cudaEvent_t ev_k0 = nullptr, ev_k1 = nullptr;   // bracket of the scan kernel
     // best-track scratch
     double *d_pool_S64 = nullptr, *d_pool_chi2 = nullptr;
     int32_t *d_pool_nmatch = nullptr;
@@ -123,6 +127,15 @@ struct cdc_events {
     double *d_wire_best = nullptr;              // [n_events][W] smallest |resid| so far
     unsigned long long *d_peak_key = nullptr;   // Hough scratch [n_events]
     int32_t max_hits_per_event = 0;
+    // matched-approach records of the re-scored candidates (A9 replays the best seed's list)
+    ApproachRec *d_rec = nullptr;               // [kRecSlots][kRecCap]
+    int32_t *d_rec_count = nullptr;             // [kRecSlots]
+    int32_t *d_pool_slot = nullptr;             // [pool_cap] record slot of a pool entry, -1 = none
+    int32_t *d_slot_counter = nullptr;
+    int32_t *d_ev_slot = nullptr;               // per event: record slot of the best seed, -1 = re-propagate
+    // one stream-ordered allocation holds every device buffer above
+    void *slab = nullptr;
+    cudaStream_t alloc_stream = nullptr;
 };
 
 enum { CNT_STEPS = 0, CNT_GAS = 1, CNT_TESTS = 2, CNT_POOL = 3, CNT_LOOKUP = 4, CNT_G1 = 5, CNT_APPROACH = 6, CNT_N = 8 };
@@ -202,6 +215,8 @@ struct BestLaunch {
     unsigned long long *d_ev_maxS, *d_ev_best;
     int32_t *d_wire_label;
     double *d_wire_best;
+    ApproachRec *d_rec;
+    int32_t *d_rec_count, *d_pool_slot, *d_slot_counter, *d_ev_slot;
     int64_t *d_best_seed;
     uint32_t *d_best_n_match;
     double *d_best_chi2;
