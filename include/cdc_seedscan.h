@@ -129,7 +129,7 @@ int32_t cdc_geometry_wire_table(const cdc_geometry *g, float *h_wire_or_null, in
  * BJ north_star: "hits binned by (layer, phi-cell) so each step's lookup is O(1)").
  * h_hit_offsets: host, n_events + 1 prefix offsets into wire_id / drift_mm.  wire_id / drift_mm live on the
  * host (hits_on_device = 0) or on the device (1).  Hits need not be sorted.  Synchronises (validation result).
- * Errors: RANGE wire id outside [0, W); INVALID duplicate wire id within an event, drift < 0 or non-finite. */
+ * Errors: RANGE wire id outside [0, W); INVALID duplicate wire id within an event, drift outside [0, 8] mm (the cell half-width, BJ configs[0]) or non-finite. */
 int32_t cdc_event_upload(const cdc_geometry *g, int32_t n_events, const int32_t *h_hit_offsets,
                          const int32_t *wire_id, const float *drift_mm, int32_t hits_on_device,
                          void *stream, cdc_events **out);

@@ -95,6 +95,26 @@ extern "C" int32_t cdc_geometry_create(const cdc_geometry_desc *gd, const cdc_fi
             }
         }
     }
+    // one cos(eps) for every wire (equal |stereo|); the scan kernel folds it into constants
+    g->uz = g->wire5[4];
+    for (int w = 0; w < g->W; ++w)
+        if (g->wire5[5 * (size_t)w + 4] != g->uz) {
+            delete g;
+            CDC_FAIL(CDC_ERR_INVALID, "cdc_geometry_create: wire table must carry one u_z (equal |stereo|)");
+        }
+    // a wire outside the 2 x 2 candidate set of a vertex is at least `excl` away from it (reading C8): one layer
+    // pitch radially, or one cell along the arc at the smallest radius a candidate can be looked up from
+    g->pitch = pitch;
+    g->excl = pitch;
+    for (int j = 0; j < L; ++j)
+        g->excl = std::min(g->excl, 2.0 * M_PI * (g->r[j] - pitch) / (double)g->n_wires[j]);
+    g->excl = 0.9975 * g->excl - 0.2;
+    {
+        const double ze = g->z_half * tan_abs;
+        g->cell_max = 0.0;
+        for (int j = 0; j < L; ++j)
+            g->cell_max = std::max(g->cell_max, 2.0 * M_PI * (sqrt(g->r[j] * g->r[j] + ze * ze) + pitch) / (double)g->n_wires[j]);
+    }
     // field
     g->field = *fd;
     if (fd->kind == 1) {
@@ -109,8 +129,12 @@ extern "C" int32_t cdc_geometry_create(const cdc_geometry_desc *gd, const cdc_fi
             CDC_FAIL(CDC_ERR_RANGE, "cdc_geometry_create: field table does not cover rho <= r_out + 8, |z| <= z_half + 8");
         }
         g->field_tab.assign(fd->h_br_bz, fd->h_br_bz + (size_t)fd->nr * fd->nz * 2);
+        for (size_t i = 0; i < (size_t)fd->nr * fd->nz; ++i)
+            g->b_max = std::max(g->b_max, hypot((double)fd->h_br_bz[2 * i], (double)fd->h_br_bz[2 * i + 1]));
         g->field.h_br_bz = g->field_tab.data();
-    } else if (fd->kind != 0) {
+    } else if (fd->kind == 0) {
+        g->b_max = fabs(fd->bz_T);
+    } else {
         delete g;
         CDC_FAIL(CDC_ERR_INVALID, "cdc_geometry_create: field kind must be 0 or 1");
     }

@@ -93,7 +93,7 @@ extern "C" int32_t cdc_event_upload(const cdc_geometry *g, int32_t n_events, con
     EV_CUDA(cudaMemcpyAsync(&err, ev->d_err, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
     EV_CUDA(cudaStreamSynchronize(s));
     if (err & 1) { free_events(ev); CDC_FAIL(CDC_ERR_RANGE, "cdc_event_upload: wire id out of range"); }
-    if (err & 2) { free_events(ev); CDC_FAIL(CDC_ERR_INVALID, "cdc_event_upload: drift distance negative or non-finite"); }
+    if (err & 2) { free_events(ev); CDC_FAIL(CDC_ERR_INVALID, "cdc_event_upload: drift distance outside [0, 8] mm or non-finite"); }
     if (err & 4) { free_events(ev); CDC_FAIL(CDC_ERR_INVALID, "cdc_event_upload: duplicate wire id within an event"); }
     *out = ev;
     return CDC_OK;

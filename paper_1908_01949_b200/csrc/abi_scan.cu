@@ -172,6 +172,26 @@ extern "C" int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cd
     L.margin = (float)(p->rescore_margin > 0.0 ? p->rescore_margin : kDefaultMargin);
     L.d_n_match = d_n_match; L.d_chi2 = d_chi2; L.d_debug = d_debug; L.d_best_key = d_best_key;
     L.d_pool = ev->d_pool; L.pool_cap = ev->pool_cap; L.d_counters = ev->d_counters;
+    // lookup cadence K: a wire that can own a match in interval n + i is within reach + i h of vertex n
+    {
+        const double dmax = 8.0 + p->window_mm + 0.05;           // largest matching D: drift <= 8 mm (upload check)
+        const double reach = sqrt(dmax * dmax + p->h_mm * p->h_mm) + 0.1;
+        if (reach > g->excl) CDC_FAIL(CDC_ERR_RANGE, "cdc_seed_scan: window + step too large for the 2 x 2 wire lookup");
+        int K = 1 + (int)floor((g->excl - reach) / p->h_mm);
+        K = std::max(1, std::min(K, 8));
+        L.lookup_every = K;
+        const double grow = reach + 0.2 + (K - 1) * p->h_mm;
+        const double ulo = std::max(g->r[0] - grow, 0.0), uhi = g->r[g->n_layers - 1] + grow;
+        L.u2_lo = (float)(ulo * ulo); L.u2_hi = (float)(uhi * uhi);
+        L.uz = g->uz; L.inv_uz = (float)(1.0 / (double)g->uz);
+        // a held wire lies within the 2 x 2 set of the last lookup vertex (two layer pitches x two cells) and
+        // the track has moved at most K h since: |delta| <= diag + K h; it stays held while the track crosses
+        // that neighbourhood, at most ~(diag + K h) / min|T_perp| of path -- bounded here by 4 diag
+        const double diag = hypot(2.0 * g->pitch, 2.0 * g->cell_max);
+        L.delta_max = (float)(diag + K * p->h_mm + 1.0);
+        L.b_max = (float)(1.001 * g->b_max);
+        L.hold_path = (float)(4.0 * diag + 2.0 * K * p->h_mm);
+    }
     L.max_seeds_per_event = 0;
     for (const GridDev &G : ev->h_grids) L.max_seeds_per_event = std::max<int64_t>(L.max_seeds_per_event, G.n_seeds);
     if (!ev->ev_k0) { CDC_CUDA(cudaEventCreate(&ev->ev_k0)); CDC_CUDA(cudaEventCreate(&ev->ev_k1)); }

@@ -62,6 +62,10 @@ struct cdc_geometry {
     std::vector<int32_t> n_wires, offset;
     std::vector<float> wire5;
     double z_half = 0, R0 = 0, r_out = 0;
+    double b_max = 0;                        // largest |B| of the field description
+    double cell_max = 0;                     // largest cell width (arc at the end plate)
+    double pitch = 0, excl = 0;              // layer pitch; distance below which a wire is surely in the 2 x 2 set
+    float uz = 1.f;
     cdc_field_desc field{};                  // h_br_bz replaced by field_tab.data()
     std::vector<float> field_tab;
     // device
@@ -171,6 +175,9 @@ struct ScanLaunch {
     uint32_t pool_cap;
     unsigned long long *d_counters;
     int64_t max_seeds_per_event;
+    float u2_lo, u2_hi, uz, inv_uz;  // lookup band (widened for the lookup cadence), cos(eps)
+    int32_t lookup_every;            // K: steps per layer/cell lookup
+    float delta_max, b_max, hold_path;   // largest |delta| of a held wire, largest |B|, longest path a wire stays held
 };
 cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0, cudaEvent_t k1);
 

@@ -21,7 +21,7 @@ __global__ void bin_hits(int32_t W, int32_t n_bit_words, const int32_t *offsets,
     const int w = wire_id[i];
     const float d = drift[i];
     if (w < 0 || w >= W) { atomicOr(err, 1); return; }
-    if (!(d >= 0.0f) || isinf(d)) { atomicOr(err, 2); return; }
+    if (!(d >= 0.0f) || !(d <= 8.0f)) { atomicOr(err, 2); return; }     // 0 <= drift <= 8 mm (cell half-width; BJ configs[0])
     const uint32_t bit = 1u << (w & 31);
     const uint32_t old = atomicOr(bits + (size_t)e * n_bit_words + (w >> 5), bit);
     if (old & bit) { atomicOr(err, 4); return; }     // duplicate wire id within the event

@@ -4,11 +4,17 @@
 // FMA chains; the six state components are carried as (hi, lo) pairs with a Kahan-compensated update so
 // that the position after thousands of steps stays within the 1e-3 mm parity bound.
 //
-//   PAPER.md:51      seed (theta0, z0, px0, py0, pz0) at R0                     -> seed_init()
-//   PAPER.md:55      RKN propagation (textbook Nystroem scheme, reading C5)     -> rkn_step()
-//   PAPER.md:55,:69  DCA to fired wires, sign-change ownership (reading C9)     -> score_wire()
-//   PAPER.md:65-69   Eq. (1): S = sum (1 - d^2/lambda) over matched terms       -> end of seed_scan_kernel
+//   PAPER.md:51      seed (theta0, z0, px0, py0, pz0) at R0                     -> kernel prologue
+//   PAPER.md:55      RKN propagation (textbook Nystroem scheme, reading C5)     -> step body
+//   PAPER.md:55,:69  DCA to fired wires, sign-change ownership (reading C9)     -> wire_g(), score_approach()
+//   PAPER.md:65-69   Eq. (1): S = sum (1 - d^2/lambda) over matched terms       -> kernel epilogue
 //   PAPER.md:69      lowest E (= highest S) wins                                -> packed-key atomicMax
+//
+// Scoring structure (r1b): the layer/cell lookup runs once every K steps (K from the step size: the 2 x 2
+// candidate set of a vertex stays a superset of the wires that can own an approach for K intervals, reading
+// C8); the candidates that carry a hit are compacted into up to four per-thread slots (wire id + g at the
+// current vertex), so each step evaluates g once per live wire and runs the approach code only on a sign
+// change.
 #include "cdc_internal.cuh"
 
 namespace {
@@ -28,7 +34,9 @@ struct ScanArgs {
     double kq;                 // kappa * charge
     double h6_64;              // h / 6 in fp64 (for the systematic-rounding correction)
     float lambda, inv_lambda, eloss_h;
-    int32_t max_steps;
+    float u2_lo, u2_hi;        // lookup band in u^2, widened by (K - 1) h
+    float uz, inv_uz;          // cos(eps) of the canonical wire table (one |stereo| for all layers)
+    int32_t max_steps, lookup_every;
     float margin;
     uint32_t *n_match;
     float *chi2;
@@ -92,61 +100,19 @@ __device__ __forceinline__ void comp_add(float &hi, float &lo, float d)
     hi = t;
 }
 
-struct Vertex {            // what scoring needs of a step vertex
-    float x, y, z, xl, yl, Tx, Ty, Tz;
-};
-
-// One candidate wire that has a hit: does interval n own an approach to it, and does the hit match?
-__device__ __forceinline__ void score_wire(const ScanArgs &A, const float *drift_e, int w, float uz, float inv_uz, const Vertex &v0,
-                                           const Vertex &v1, uint32_t &nm, float &chi2, uint32_t &cnt)
+// g = delta . T for wire wr = (w0x, w0y, ux, uy) at a vertex; also returns e (offset of the vertex from the wire
+// point at the vertex' own height: a horizontal vector of at most ~17 mm) and e.u.  Written with explicit
+// round-to-nearest intrinsics only: the value of g at a vertex must not depend on the call site (it is evaluated
+// once as the far end of interval n - 1 or at a lookup, and reused as the near end of interval n).
+__device__ __forceinline__ float wire_g(const float4 wr, float uz, float inv_uz, float x, float xl, float y, float yl,
+                                        float z, float Tx, float Ty, float Tz, float &ex, float &ey, float &eu)
 {
-    float4 wr = __ldg(A.gd.wire4 + w);
-    float zt0 = v0.z * inv_uz;
-    float ex0 = fmaf(-zt0, wr.z, v0.x - wr.x) + v0.xl;     // offset from the wire point at the vertex' height
-    float ey0 = fmaf(-zt0, wr.w, v0.y - wr.y) + v0.yl;
-    float uT0 = fmaf(wr.z, v0.Tx, fmaf(wr.w, v0.Ty, uz * v0.Tz));
-    float eu0 = fmaf(ex0, wr.z, ey0 * wr.w);
-    float g0 = fmaf(ex0, v0.Tx, fmaf(ey0, v0.Ty, -eu0 * uT0));   // g = delta . T, delta = e - (e.u) u
-    if (!(g0 <= 0.0f)) return;
-    cnt += 1u;                                                // packed: g1 evaluations | owned approaches << 16
-    float zt1 = v1.z * inv_uz;
-    float ex1 = fmaf(-zt1, wr.z, v1.x - wr.x) + v1.xl;
-    float ey1 = fmaf(-zt1, wr.w, v1.y - wr.y) + v1.yl;
-    float uT1 = fmaf(wr.z, v1.Tx, fmaf(wr.w, v1.Ty, uz * v1.Tz));
-    float eu1 = fmaf(ex1, wr.z, ey1 * wr.w);
-    float g1 = fmaf(ex1, v1.Tx, fmaf(ey1, v1.Ty, -eu1 * uT1));
-    if (!(g1 > 0.0f)) return;
-    cnt += 1u << 16;
-    float tau = __fdividef(g0, g0 - g1);
-    float ex = fmaf(tau, ex1 - ex0, ex0);                   // e is linear in the position: exact chord point
-    float ey = fmaf(tau, ey1 - ey0, ey0);
-    float eu = fmaf(ex, wr.z, ey * wr.w);
-    float D2 = fmaf(ex, ex, fmaf(ey, ey, -eu * eu));
-    float D = sqrtf(fmaxf(D2, 0.0f));
-    float zP = fmaf(tau, v1.z - v0.z, v0.z);
-    float zw = fmaf(eu, uz, zP);
-    float resid = D - __ldg(drift_e + w);
-    float r2 = resid * resid;
-    if (fabsf(zw) <= A.gd.z_half && r2 < A.lambda) { nm += 1u; chi2 += r2; }
-}
-
-__device__ __forceinline__ void score_layer(const ScanArgs &A, const float *drift_e, const LayerDev *s_layer, const uint32_t *s_bits,
-                                            int j, float phi, const Vertex &v0, const Vertex &v1, uint32_t &nm,
-                                            float &chi2, uint32_t &tests, uint32_t &cnt)
-{
-    if ((unsigned)j >= (unsigned)A.gd.n_layers) return;
-    const LayerDev L = s_layer[j];
-    float tau = v0.z * L.shift_k;
-    float sh = fmaf(-0.333333343f * tau * tau, tau, tau);      // atan(tau), |tau| < 0.1
-    float kf = (phi - L.phi0 - sh) * L.kscale;
-    float kn = rintf(kf);
-    int k1 = (int)kn;
-    int k2 = k1 + ((kf - kn) >= 0.0f ? 1 : -1);
-    k1 += (k1 < 0) ? L.n : 0; k1 += (k1 < 0) ? L.n : 0; k1 -= (k1 >= L.n) ? L.n : 0;
-    k2 += (k2 < 0) ? L.n : 0; k2 += (k2 < 0) ? L.n : 0; k2 -= (k2 >= L.n) ? L.n : 0;
-    int w1 = L.offset + k1, w2 = L.offset + k2;
-    if ((s_bits[w1 >> 5] >> (w1 & 31)) & 1u) { tests += 1u; score_wire(A, drift_e, w1, L.uz, L.inv_uz, v0, v1, nm, chi2, cnt); }
-    if ((s_bits[w2 >> 5] >> (w2 & 31)) & 1u) { tests += 1u; score_wire(A, drift_e, w2, L.uz, L.inv_uz, v0, v1, nm, chi2, cnt); }
+    const float zt = __fmul_rn(z, inv_uz);
+    ex = __fadd_rn(__fmaf_rn(-zt, wr.z, __fsub_rn(x, wr.x)), xl);
+    ey = __fadd_rn(__fmaf_rn(-zt, wr.w, __fsub_rn(y, wr.y)), yl);
+    const float uT = __fmaf_rn(wr.z, Tx, __fmaf_rn(wr.w, Ty, __fmul_rn(uz, Tz)));
+    eu = __fmaf_rn(ex, wr.z, __fmul_rn(ey, wr.w));
+    return __fmaf_rn(ex, Tx, __fmaf_rn(ey, Ty, -__fmul_rn(eu, uT)));
 }
 
 __device__ __forceinline__ unsigned long long warp_max_u64(unsigned long long v)
@@ -157,6 +123,69 @@ __device__ __forceinline__ unsigned long long warp_max_u64(unsigned long long v)
         v = other > v ? other : v;
     }
     return v;
+}
+
+struct Slots {             // live candidate wires of this thread (those that carry a hit), and g at the current vertex
+    int w0, w1, w2, w3;
+    float g0, g1, g2, g3;
+    int n;
+};
+
+__device__ __forceinline__ void slot_push(Slots &S, int w)
+{
+    if (S.n == 0) S.w0 = w; else if (S.n == 1) S.w1 = w; else if (S.n == 2) S.w2 = w; else S.w3 = w;
+    S.n += 1;
+}
+
+// cells kc and its nearer neighbour of layer j around azimuth phi at height z -> push those with a hit
+__device__ __forceinline__ void lookup_layer(const LayerDev *s_layer, const uint32_t *s_bits, int n_layers, int j,
+                                             float phi, float z, Slots &S)
+{
+    if ((unsigned)j >= (unsigned)n_layers) return;
+    const LayerDev L = s_layer[j];
+    const float tau = z * L.shift_k;
+    const float sh = fmaf(-0.333333343f * tau * tau, tau, tau);      // atan(tau), |tau| < 0.1
+    const float kf = (phi - L.phi0 - sh) * L.kscale;
+    const float kn = rintf(kf);
+    int k1 = (int)kn;
+    int k2 = k1 + ((kf - kn) >= 0.0f ? 1 : -1);
+    k1 += (k1 < 0) ? L.n : 0; k1 += (k1 < 0) ? L.n : 0; k1 -= (k1 >= L.n) ? L.n : 0;
+    k2 += (k2 < 0) ? L.n : 0; k2 += (k2 < 0) ? L.n : 0; k2 -= (k2 >= L.n) ? L.n : 0;
+    const int w1 = L.offset + k1, w2 = L.offset + k2;
+    if ((s_bits[w1 >> 5] >> (w1 & 31)) & 1u) slot_push(S, w1);
+    if ((s_bits[w2 >> 5] >> (w2 & 31)) & 1u) slot_push(S, w2);
+}
+
+struct Vtx {               // position part of a step vertex (hi + the lo of x, y that the wire offset uses)
+    float x, xl, y, yl, z;
+};
+
+// One live wire over interval n: g at the far vertex; on g_n <= 0 < g_{n+1} the interval owns an approach (C9).
+__device__ __forceinline__ void slot_step(const ScanArgs &A, const float *drift_e, int w, float &g, bool score,
+                                          const Vtx &v0, const Vtx &v1, float Tx1, float Ty1, float Tz1,
+                                          uint32_t &nm, float &chi2, uint32_t &cnt)
+{
+    const float4 wr = __ldg(A.gd.wire4 + w);
+    float ex1, ey1, eu1;
+    const float gn = wire_g(wr, A.uz, A.inv_uz, v1.x, v1.xl, v1.y, v1.yl, v1.z, Tx1, Ty1, Tz1, ex1, ey1, eu1);
+    if (score && g <= 0.0f && gn > 0.0f) {
+        cnt += 1u << 16;
+        const float zt0 = __fmul_rn(v0.z, A.inv_uz);
+        const float ex0 = __fadd_rn(__fmaf_rn(-zt0, wr.z, __fsub_rn(v0.x, wr.x)), v0.xl);
+        const float ey0 = __fadd_rn(__fmaf_rn(-zt0, wr.w, __fsub_rn(v0.y, wr.y)), v0.yl);
+        const float tau = __fdividef(g, g - gn);
+        const float ex = fmaf(tau, ex1 - ex0, ex0);            // e is linear in the position: exact chord point
+        const float ey = fmaf(tau, ey1 - ey0, ey0);
+        const float eu = fmaf(ex, wr.z, ey * wr.w);
+        const float D2 = fmaf(ex, ex, fmaf(ey, ey, -eu * eu));
+        const float D = sqrtf(fmaxf(D2, 0.0f));
+        const float zP = fmaf(tau, v1.z - v0.z, v0.z);
+        const float zw = fmaf(eu, A.uz, zP);
+        const float resid = D - __ldg(drift_e + w);
+        const float r2 = resid * resid;
+        if (fabsf(zw) <= A.gd.z_half && r2 < A.lambda) { nm += 1u; chi2 += r2; }
+    }
+    g = gn;
 }
 
 template <int FIELD, bool ELOSS>
@@ -209,69 +238,108 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
 
     uint32_t nm = 0, tests = 0, cnt = 0, lookups = 0;
     float chi2 = 0.0f;
-    int n = 0, m = 0, turn = 0;
+    int n = 0, m = 0, turn = 0, kcount = 0;
     bool cn = true;                                   // c_0 := true (reading C7)
     const float h = A.h;
+    Slots S;
+    S.n = 0; S.w0 = S.w1 = S.w2 = S.w3 = 0; S.g0 = S.g1 = S.g2 = S.g3 = 0.0f;
 
     while (valid && n < A.max_steps) {
-        Vertex v0;
-        v0.x = xh; v0.y = yh; v0.z = zh; v0.xl = xl; v0.yl = yl; v0.Tx = Txh; v0.Ty = Tyh; v0.Tz = Tzh;
+        // ---- A5: every K steps, the wires near r_n that carry a hit -> slots, with g at this vertex
+        if (kcount == 0) {
+            kcount = A.lookup_every;
+            S.n = 0;
+            const float zeta = zh * A.gd.tan_abs;
+            const float u2 = fmaf(xh, xh, fmaf(yh, yh, -zeta * zeta));
+            if (u2 > A.u2_lo && u2 < A.u2_hi) {
+                lookups += 1u;
+                const float u = u2 * rsqrtf(u2);
+                const float fj = (u - A.gd.r_first) * A.gd.inv_pitch;
+                const float jn = rintf(fj);
+                const int jc = (int)jn;
+                const int j2 = jc + ((fj - jn) >= 0.0f ? 1 : -1);
+                const float phi = coarse_atan2(yh, xh);
+                lookup_layer(s_layer, s_bits, A.gd.n_layers, jc, phi, zh, S);
+                lookup_layer(s_layer, s_bits, A.gd.n_layers, j2, phi, zh, S);
+                float ex, ey, eu;
+                cnt += (uint32_t)S.n;
+                if (S.n > 0) S.g0 = wire_g(__ldg(A.gd.wire4 + S.w0), A.uz, A.inv_uz, xh, xl, yh, yl, zh, Txh, Tyh, Tzh, ex, ey, eu);
+                if (S.n > 1) S.g1 = wire_g(__ldg(A.gd.wire4 + S.w1), A.uz, A.inv_uz, xh, xl, yh, yl, zh, Txh, Tyh, Tzh, ex, ey, eu);
+                if (S.n > 2) S.g2 = wire_g(__ldg(A.gd.wire4 + S.w2), A.uz, A.inv_uz, xh, xl, yh, yl, zh, Txh, Tyh, Tzh, ex, ey, eu);
+                if (S.n > 3) S.g3 = wire_g(__ldg(A.gd.wire4 + S.w3), A.uz, A.inv_uz, xh, xl, yh, yl, zh, Txh, Tyh, Tzh, ex, ey, eu);
+            }
+        }
+        kcount -= 1;
+        Vtx v0;
+        v0.x = xh; v0.xl = xl; v0.y = yh; v0.yl = yl; v0.z = zh;
 
         // ---- A4: one Nystroem-RK4 step of r'' = a (r' x B(r))
-        float Bx, By, Bz;
-        field_at<FIELD>(A.fd, xh, yh, zh, Bx, By, Bz);
-        float k1x = a * fmaf(Tyh, Bz, -Tzh * By), k1y = a * fmaf(Tzh, Bx, -Txh * Bz), k1z = a * fmaf(Txh, By, -Tyh * Bx);
-        float Ux = fmaf(A.h_half, k1x, Txh), Uy = fmaf(A.h_half, k1y, Tyh), Uz = fmaf(A.h_half, k1z, Tzh);
-        if (FIELD != 0) {
-            float mx = fmaf(A.h2_8, k1x, fmaf(A.h_half, Txh, xh));
-            float my = fmaf(A.h2_8, k1y, fmaf(A.h_half, Tyh, yh));
-            float mz = fmaf(A.h2_8, k1z, fmaf(A.h_half, Tzh, zh));
-            field_at<FIELD>(A.fd, mx, my, mz, Bx, By, Bz);
-        }
-        float k2x = a * fmaf(Uy, Bz, -Uz * By), k2y = a * fmaf(Uz, Bx, -Ux * Bz), k2z = a * fmaf(Ux, By, -Uy * Bx);
-        Ux = fmaf(A.h_half, k2x, Txh); Uy = fmaf(A.h_half, k2y, Tyh); Uz = fmaf(A.h_half, k2z, Tzh);
-        float k3x = a * fmaf(Uy, Bz, -Uz * By), k3y = a * fmaf(Uz, Bx, -Ux * Bz), k3z = a * fmaf(Ux, By, -Uy * Bx);
-        Ux = fmaf(h, k3x, Txh); Uy = fmaf(h, k3y, Tyh); Uz = fmaf(h, k3z, Tzh);
-        if (FIELD != 0) {
-            float ex = fmaf(A.h2_2, k3x, fmaf(h, Txh, xh));
-            float ey = fmaf(A.h2_2, k3y, fmaf(h, Tyh, yh));
-            float ez = fmaf(A.h2_2, k3z, fmaf(h, Tzh, zh));
-            field_at<FIELD>(A.fd, ex, ey, ez, Bx, By, Bz);
-        }
-        float k4x = a * fmaf(Uy, Bz, -Uz * By), k4y = a * fmaf(Uz, Bx, -Ux * Bz), k4z = a * fmaf(Ux, By, -Uy * Bx);
-
-        float dx = fmaf(A.h2_6, (k1x + k2x) + k3x, h * Txh);
-        float dy = fmaf(A.h2_6, (k1y + k2y) + k3y, h * Tyh);
-        float dz = fmaf(A.h2_6, (k1z + k2z) + k3z, h * Tzh);
-        float dTx = A.h_6 * ((k1x + k4x) + 2.0f * (k2x + k3x));
-        float dTy = A.h_6 * ((k1y + k4y) + 2.0f * (k2y + k3y));
-        float dTz = A.h_6 * ((k1z + k4z) + 2.0f * (k2z + k3z));
-        comp_add(xh, xl, fmaf(h, Txl, dx));            // h * T_lo: the part of T the fp32 stages never saw
-        comp_add(yh, yl, fmaf(h, Tyl, dy));
-        comp_add(zh, zl, fmaf(h, Tzl, dz));
-        comp_add(Txh, Txl, fmaf(dTx, epsT, dTx));
-        comp_add(Tyh, Tyl, fmaf(dTy, epsT, dTy));
-        if (FIELD != 0) comp_add(Tzh, Tzl, fmaf(dTz, epsT, dTz));   // uniform field: k_z == 0, T_z is constant
-
-        // ---- A5/A6: wires near r_n, owned approaches, score (only if the interval starts in the gas)
-        if (cn) {
-            float zeta = v0.z * A.gd.tan_abs;
-            float u2 = fmaf(v0.x, v0.x, fmaf(v0.y, v0.y, -zeta * zeta));
-            if (u2 > A.gd.u2_lo && u2 < A.gd.u2_hi) {
-                Vertex v1;
-                v1.x = xh; v1.y = yh; v1.z = zh; v1.xl = xl; v1.yl = yl; v1.Tx = Txh; v1.Ty = Tyh; v1.Tz = Tzh;
-                lookups += 1u;
-                float u = u2 * rsqrtf(u2);
-                float fj = (u - A.gd.r_first) * A.gd.inv_pitch;
-                float jn = rintf(fj);
-                int jc = (int)jn;
-                int j2 = jc + ((fj - jn) >= 0.0f ? 1 : -1);
-                float phi = coarse_atan2(v0.y, v0.x);
-                score_layer(A, drift_e, s_layer, s_bits, jc, phi, v0, v1, nm, chi2, tests, cnt);
-                score_layer(A, drift_e, s_layer, s_bits, j2, phi, v0, v1, nm, chi2, tests, cnt);
+        if (FIELD == 0) {
+            // uniform field B = (0, 0, Bz): k = a Bz (T_y, -T_x, 0); k_z == 0, T_z constant, no stage positions needed
+            const float c = a * A.fd.bz;
+            const float k1x = c * Tyh, k1y = -c * Txh;
+            float Ux = fmaf(A.h_half, k1x, Txh), Uy = fmaf(A.h_half, k1y, Tyh);
+            const float k2x = c * Uy, k2y = -c * Ux;
+            Ux = fmaf(A.h_half, k2x, Txh); Uy = fmaf(A.h_half, k2y, Tyh);
+            const float k3x = c * Uy, k3y = -c * Ux;
+            Ux = fmaf(h, k3x, Txh); Uy = fmaf(h, k3y, Tyh);
+            const float k4x = c * Uy, k4y = -c * Ux;
+            const float dx = fmaf(A.h2_6, (k1x + k2x) + k3x, h * Txh);
+            const float dy = fmaf(A.h2_6, (k1y + k2y) + k3y, h * Tyh);
+            const float dTx = A.h_6 * fmaf(2.0f, k2x + k3x, k1x + k4x);
+            const float dTy = A.h_6 * fmaf(2.0f, k2y + k3y, k1y + k4y);
+            comp_add(xh, xl, fmaf(h, Txl, dx));        // h * T_lo: the part of T the fp32 stages never saw
+            comp_add(yh, yl, fmaf(h, Tyl, dy));
+            comp_add(zh, zl, fmaf(h, Tzl, h * Tzh));
+            comp_add(Txh, Txl, fmaf(dTx, epsT, dTx));
+            comp_add(Tyh, Tyl, fmaf(dTy, epsT, dTy));
+        } else {
+            float Bx, By, Bz;
+            field_at<FIELD>(A.fd, xh, yh, zh, Bx, By, Bz);
+            const float k1x = a * fmaf(Tyh, Bz, -Tzh * By), k1y = a * fmaf(Tzh, Bx, -Txh * Bz), k1z = a * fmaf(Txh, By, -Tyh * Bx);
+            float Ux = fmaf(A.h_half, k1x, Txh), Uy = fmaf(A.h_half, k1y, Tyh), Uz = fmaf(A.h_half, k1z, Tzh);
+            {
+                const float mx = fmaf(A.h2_8, k1x, fmaf(A.h_half, Txh, xh));
+                const float my = fmaf(A.h2_8, k1y, fmaf(A.h_half, Tyh, yh));
+                const float mz = fmaf(A.h2_8, k1z, fmaf(A.h_half, Tzh, zh));
+                field_at<FIELD>(A.fd, mx, my, mz, Bx, By, Bz);
             }
-            m += 1;
+            const float k2x = a * fmaf(Uy, Bz, -Uz * By), k2y = a * fmaf(Uz, Bx, -Ux * Bz), k2z = a * fmaf(Ux, By, -Uy * Bx);
+            Ux = fmaf(A.h_half, k2x, Txh); Uy = fmaf(A.h_half, k2y, Tyh); Uz = fmaf(A.h_half, k2z, Tzh);
+            const float k3x = a * fmaf(Uy, Bz, -Uz * By), k3y = a * fmaf(Uz, Bx, -Ux * Bz), k3z = a * fmaf(Ux, By, -Uy * Bx);
+            Ux = fmaf(h, k3x, Txh); Uy = fmaf(h, k3y, Tyh); Uz = fmaf(h, k3z, Tzh);
+            {
+                const float ex = fmaf(A.h2_2, k3x, fmaf(h, Txh, xh));
+                const float ey = fmaf(A.h2_2, k3y, fmaf(h, Tyh, yh));
+                const float ez = fmaf(A.h2_2, k3z, fmaf(h, Tzh, zh));
+                field_at<FIELD>(A.fd, ex, ey, ez, Bx, By, Bz);
+            }
+            const float k4x = a * fmaf(Uy, Bz, -Uz * By), k4y = a * fmaf(Uz, Bx, -Ux * Bz), k4z = a * fmaf(Ux, By, -Uy * Bx);
+            const float dx = fmaf(A.h2_6, (k1x + k2x) + k3x, h * Txh);
+            const float dy = fmaf(A.h2_6, (k1y + k2y) + k3y, h * Tyh);
+            const float dz = fmaf(A.h2_6, (k1z + k2z) + k3z, h * Tzh);
+            const float dTx = A.h_6 * fmaf(2.0f, k2x + k3x, k1x + k4x);
+            const float dTy = A.h_6 * fmaf(2.0f, k2y + k3y, k1y + k4y);
+            const float dTz = A.h_6 * fmaf(2.0f, k2z + k3z, k1z + k4z);
+            comp_add(xh, xl, fmaf(h, Txl, dx));
+            comp_add(yh, yl, fmaf(h, Tyl, dy));
+            comp_add(zh, zl, fmaf(h, Tzl, dz));
+            comp_add(Txh, Txl, fmaf(dTx, epsT, dTx));
+            comp_add(Tyh, Tyl, fmaf(dTy, epsT, dTy));
+            comp_add(Tzh, Tzl, fmaf(dTz, epsT, dTz));
         }
+
+        // ---- A6: live wires over interval n (scored only if the interval starts in the gas)
+        if (S.n > 0) {
+            Vtx v1;
+            v1.x = xh; v1.xl = xl; v1.y = yh; v1.yl = yl; v1.z = zh;
+            tests += (uint32_t)S.n;
+            slot_step(A, drift_e, S.w0, S.g0, cn, v0, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
+            if (S.n > 1) slot_step(A, drift_e, S.w1, S.g1, cn, v0, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
+            if (S.n > 2) slot_step(A, drift_e, S.w2, S.g2, cn, v0, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
+            if (S.n > 3) slot_step(A, drift_e, S.w3, S.g3, cn, v0, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
+        }
+        if (cn) m += 1;
 
         // ---- advance, energy loss (reading C6), turn counter and termination (reading C7)
         n += 1;
@@ -290,7 +358,7 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
     }
 
     // ---- A7: per-seed output, per-event argmax, candidate pool
-    const float S = valid ? fmaf(-chi2, A.inv_lambda, (float)nm) : -1.0f;
+    const float S32 = valid ? fmaf(-chi2, A.inv_lambda, (float)nm) : -1.0f;
     if (valid) {
         const int64_t o = G.out_offset + (int64_t)index;
         if (A.n_match) A.n_match[o] = nm;
@@ -302,7 +370,7 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
             A.debug[o] = d;
         }
     }
-    const float Sc = fmaxf(S, 0.0f);                  // S >= 0 by construction; clamp rounding residue
+    const float Sc = fmaxf(S32, 0.0f);                // S >= 0 by construction; clamp rounding residue
     unsigned long long key = valid ? (((unsigned long long)__float_as_uint(Sc) << 32) | (0xFFFFFFFFu - index)) : 0ull;
     unsigned long long wkey = warp_max_u64(key);
     const int lane = threadIdx.x & 31;
@@ -355,11 +423,12 @@ cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0
     A.h_6 = (float)(h / 6.0); A.h2_6 = (float)(h * h / 6.0);
     A.kq = CDC_KAPPA * (double)L.charge; A.h6_64 = h / 6.0;
     A.lambda = L.lambda; A.inv_lambda = 1.0f / L.lambda; A.eloss_h = L.eloss_h;
+    A.u2_lo = L.u2_lo; A.u2_hi = L.u2_hi; A.uz = L.uz; A.inv_uz = L.inv_uz; A.lookup_every = L.lookup_every;
     A.max_steps = L.max_steps; A.margin = L.margin;
     A.n_match = L.d_n_match; A.chi2 = L.d_chi2; A.debug = L.d_debug;
     A.best_key = (unsigned long long *)L.d_best_key;
     A.pool = L.d_pool; A.pool_cap = L.pool_cap; A.counters = L.d_counters;
-    if (L.gd.n_bit_words > kMaxBitWords || L.gd.n_layers > CDC_MAX_LAYERS) return cudaErrorInvalidValue;
+    if (L.gd.n_bit_words > kMaxBitWords || L.gd.n_layers > CDC_MAX_LAYERS || L.lookup_every < 1) return cudaErrorInvalidValue;
     dim3 grid((unsigned)((L.max_seeds_per_event + kBlock - 1) / kBlock), (unsigned)L.n_events);
     const bool eloss = L.eloss_h != 0.0f;
     if (k0) cudaEventRecord(k0, s);
