@@ -36,6 +36,7 @@ struct ScanArgs {
     float lambda, inv_lambda, eloss_h;
     float u2_lo, u2_hi;        // lookup band in u^2, widened by (K - 1) h
     float uz, inv_uz;          // cos(eps) of the canonical wire table (one |stereo| for all layers)
+    float delta_max, b_max, hold_path;   // bounds behind g_dead (see consider())
     int32_t max_steps, lookup_every;
     float margin;
     uint32_t *n_match;
@@ -131,18 +132,36 @@ struct Slots {             // live candidate wires of this thread (those that ca
     int n;
 };
 
-__device__ __forceinline__ void slot_push(Slots &S, int w)
+__device__ __forceinline__ void slot_push(Slots &S, int w, float g)
 {
-    if (S.n == 0) S.w0 = w; else if (S.n == 1) S.w1 = w; else if (S.n == 2) S.w2 = w; else S.w3 = w;
+    if (S.n == 0) { S.w0 = w; S.g0 = g; } else if (S.n == 1) { S.w1 = w; S.g1 = g; }
+    else if (S.n == 2) { S.w2 = w; S.g2 = g; } else { S.w3 = w; S.g3 = g; }
     S.n += 1;
 }
 
-// cells kc and its nearer neighbour of layer j around azimuth phi at height z -> push those with a hit
-__device__ __forceinline__ void lookup_layer(const LayerDev *s_layer, const uint32_t *s_bits, int n_layers, int j,
-                                             float phi, float z, Slots &S)
+struct LookupCtx {         // the vertex a lookup is made from
+    float x, xl, y, yl, z, Tx, Ty, Tz, phi, g_dead;
+};
+
+// a candidate with a hit becomes a live slot unless the track has already passed it for good: once g exceeds
+// g_dead it cannot return to <= 0 while the wire is in reach (g' >= |T_perp|^2 - |delta| |T'| >= -(|delta| |a| B)^2 / 4)
+__device__ __forceinline__ void consider(const ScanArgs &A, const uint32_t *s_bits, int w, const LookupCtx &V, Slots &S,
+                                         uint32_t &cnt)
 {
-    if ((unsigned)j >= (unsigned)n_layers) return;
+    if (!((s_bits[w >> 5] >> (w & 31)) & 1u)) return;
+    float ex, ey, eu;
+    cnt += 1u;
+    const float g = wire_g(__ldg(A.gd.wire4 + w), A.uz, A.inv_uz, V.x, V.xl, V.y, V.yl, V.z, V.Tx, V.Ty, V.Tz, ex, ey, eu);
+    if (g <= V.g_dead) slot_push(S, w, g);
+}
+
+// cells kc and its nearer neighbour of layer j around azimuth phi at height z -> push those with a hit
+__device__ __forceinline__ void lookup_layer(const ScanArgs &A, const LayerDev *s_layer, const uint32_t *s_bits, int j,
+                                             const LookupCtx &V, Slots &S, uint32_t &cnt)
+{
+    if ((unsigned)j >= (unsigned)A.gd.n_layers) return;
     const LayerDev L = s_layer[j];
+    const float phi = V.phi, z = V.z;
     const float tau = z * L.shift_k;
     const float sh = fmaf(-0.333333343f * tau * tau, tau, tau);      // atan(tau), |tau| < 0.1
     const float kf = (phi - L.phi0 - sh) * L.kscale;
@@ -151,9 +170,8 @@ __device__ __forceinline__ void lookup_layer(const LayerDev *s_layer, const uint
     int k2 = k1 + ((kf - kn) >= 0.0f ? 1 : -1);
     k1 += (k1 < 0) ? L.n : 0; k1 += (k1 < 0) ? L.n : 0; k1 -= (k1 >= L.n) ? L.n : 0;
     k2 += (k2 < 0) ? L.n : 0; k2 += (k2 < 0) ? L.n : 0; k2 -= (k2 >= L.n) ? L.n : 0;
-    const int w1 = L.offset + k1, w2 = L.offset + k2;
-    if ((s_bits[w1 >> 5] >> (w1 & 31)) & 1u) slot_push(S, w1);
-    if ((s_bits[w2 >> 5] >> (w2 & 31)) & 1u) slot_push(S, w2);
+    consider(A, s_bits, L.offset + k1, V, S, cnt);
+    consider(A, s_bits, L.offset + k2, V, S, cnt);
 }
 
 struct Vtx {               // position part of a step vertex (hi + the lo of x, y that the wire offset uses)
@@ -244,6 +262,7 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
     Slots S;
     S.n = 0; S.w0 = S.w1 = S.w2 = S.w3 = 0; S.g0 = S.g1 = S.g2 = S.g3 = 0.0f;
 
+#pragma unroll 2
     while (valid && n < A.max_steps) {
         // ---- A5: every K steps, the wires near r_n that carry a hit -> slots, with g at this vertex
         if (kcount == 0) {
@@ -258,15 +277,15 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
                 const float jn = rintf(fj);
                 const int jc = (int)jn;
                 const int j2 = jc + ((fj - jn) >= 0.0f ? 1 : -1);
-                const float phi = coarse_atan2(yh, xh);
-                lookup_layer(s_layer, s_bits, A.gd.n_layers, jc, phi, zh, S);
-                lookup_layer(s_layer, s_bits, A.gd.n_layers, j2, phi, zh, S);
-                float ex, ey, eu;
-                cnt += (uint32_t)S.n;
-                if (S.n > 0) S.g0 = wire_g(__ldg(A.gd.wire4 + S.w0), A.uz, A.inv_uz, xh, xl, yh, yl, zh, Txh, Tyh, Tzh, ex, ey, eu);
-                if (S.n > 1) S.g1 = wire_g(__ldg(A.gd.wire4 + S.w1), A.uz, A.inv_uz, xh, xl, yh, yl, zh, Txh, Tyh, Tzh, ex, ey, eu);
-                if (S.n > 2) S.g2 = wire_g(__ldg(A.gd.wire4 + S.w2), A.uz, A.inv_uz, xh, xl, yh, yl, zh, Txh, Tyh, Tzh, ex, ey, eu);
-                if (S.n > 3) S.g3 = wire_g(__ldg(A.gd.wire4 + S.w3), A.uz, A.inv_uz, xh, xl, yh, yl, zh, Txh, Tyh, Tzh, ex, ey, eu);
+                LookupCtx V;
+                V.x = xh; V.xl = xl; V.y = yh; V.yl = yl; V.z = zh; V.Tx = Txh; V.Ty = Tyh; V.Tz = Tzh;
+                V.phi = coarse_atan2(yh, xh);
+                {
+                    const float cbend = (ELOSS ? 1.05f : 1.0f) * A.delta_max * fabsf(a) * A.b_max;
+                    V.g_dead = fmaf(A.hold_path * 0.25f, cbend * cbend, 0.02f);
+                }
+                lookup_layer(A, s_layer, s_bits, jc, V, S, cnt);
+                lookup_layer(A, s_layer, s_bits, j2, V, S, cnt);
             }
         }
         kcount -= 1;
@@ -424,6 +443,7 @@ cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0
     A.kq = CDC_KAPPA * (double)L.charge; A.h6_64 = h / 6.0;
     A.lambda = L.lambda; A.inv_lambda = 1.0f / L.lambda; A.eloss_h = L.eloss_h;
     A.u2_lo = L.u2_lo; A.u2_hi = L.u2_hi; A.uz = L.uz; A.inv_uz = L.inv_uz; A.lookup_every = L.lookup_every;
+    A.delta_max = L.delta_max; A.b_max = L.b_max; A.hold_path = L.hold_path;
     A.max_steps = L.max_steps; A.margin = L.margin;
     A.n_match = L.d_n_match; A.chi2 = L.d_chi2; A.debug = L.d_debug;
     A.best_key = (unsigned long long *)L.d_best_key;
