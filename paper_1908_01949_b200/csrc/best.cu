@@ -90,46 +90,42 @@ __device__ __forceinline__ void wire_offset64(const float *w, const double *r, d
     *tpar = t;
 }
 
-// candidate wires around r: 3 nearest layers x 3 nearest cells, those with a hit, ascending wire id
-// (fp32 is enough: the set only has to contain every wire within ~9.3 mm, reading C8)
-__device__ int candidates64(const Geom64 &g, const uint32_t *bits, const double *r, int *cand)
-{
-    const float x = (float)r[0], y = (float)r[1], z = (float)r[2];
-    const float zeta = z * g.tan_abs;
-    const float u2 = x * x + y * y - zeta * zeta;
-    if (!(u2 > 0.0f)) return 0;
-    const float fj = (sqrtf(u2) - g.r_first) * g.inv_pitch;
-    if (fj < -1.0f || fj > (float)g.n_layers) return 0;
-    const int jc = (int)rintf(fj);
-    const float phi = atan2f(y, x);
-    int n = 0;
-    for (int j = jc - 1; j <= jc + 1; ++j) {
-        if (j < 0 || j >= g.n_layers) continue;
-        const LayerDev L = g.layers[j];
-        const float kf = (phi - L.phi0 - atanf(z * L.shift_k)) * L.kscale;
-        const int kc = (int)rintf(kf);
-        for (int dk = -1; dk <= 1; ++dk) {
-            int k = kc + dk;                                         // |k| < 2 n: wrap without a division
-            k += (k < 0) ? L.n : 0; k += (k < 0) ? L.n : 0; k -= (k >= L.n) ? L.n : 0;
-            const int w = L.offset + k;
-            if (!((bits[w >> 5] >> (w & 31)) & 1u)) continue;
-            int i = n++;
-            while (i > 0 && cand[i - 1] > w) { cand[i] = cand[i - 1]; --i; }   // insertion sort, ascending id
-            cand[i] = w;
-        }
-    }
-    return n;
-}
-
 struct Eval64 {
     int32_t n_match, n_steps, turns, m_gas;
     double chi2;
 };
 
-// readings C4-C10: evaluate one seed.  wire_label / wire_best (optional, per wire of this event): reading C12.
-__device__ void eval_seed64(const BestArgs &A, int e, uint32_t index, Eval64 &out, int32_t *wire_label,
-                            double *wire_best, ApproachRec *rec, int32_t *rec_count)
+// this lane's candidate wire around r, or -1: lanes 0..8 cover the 3 nearest layers x 3 nearest cells; only wires
+// with a hit are returned (fp32 is enough here: the set only has to contain every wire within ~9.3 mm, reading C8)
+__device__ __forceinline__ int lane_candidate(const Geom64 &g, const LayerDev *s_layer, const uint32_t *bits,
+                                              const double *r, int lane)
 {
+    const float x = (float)r[0], y = (float)r[1], z = (float)r[2];
+    const float zeta = z * g.tan_abs;
+    const float u2 = x * x + y * y - zeta * zeta;
+    if (!(u2 > 0.0f) || lane >= 9) return -1;
+    const float fj = (sqrtf(u2) - g.r_first) * g.inv_pitch;
+    if (fj < -1.0f || fj > (float)g.n_layers) return -1;
+    const int j = (int)rintf(fj) - 1 + lane / 3;
+    if (j < 0 || j >= g.n_layers) return -1;
+    const LayerDev L = s_layer[j];
+    const float kf = (atan2f(y, x) - L.phi0 - atanf(z * L.shift_k)) * L.kscale;
+    int k = (int)rintf(kf) + (lane % 3) - 1;                         // |k| < 2 n: wrap without a division
+    k += (k < 0) ? L.n : 0; k += (k < 0) ? L.n : 0; k -= (k >= L.n) ? L.n : 0;
+    const int w = L.offset + k;
+    return ((__ldg(bits + (w >> 5)) >> (w & 31)) & 1u) ? w : -1;
+}
+
+// readings C4-C10: evaluate one seed, one WARP per seed.  Every lane carries the same fp64 track (the arithmetic is
+// redundant across lanes, which costs nothing: the warp issues it once); lanes 0..8 each test one candidate wire of
+// the interval, so the latency of a step is that of one wire instead of nine.  Matches are folded into chi2 in
+// ascending wire id within an interval -- the order reading C11 fixes.  wire_label / wire_best (optional, per wire
+// of this event): reading C12.  rec / rec_count (optional): matched approaches in path order.
+__device__ void eval_seed64(const BestArgs &A, const LayerDev *s_layer, int e, uint32_t index, Eval64 &out,
+                            int32_t *wire_label, double *wire_best, ApproachRec *rec, int32_t *rec_count)
+{
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
     const GridDev G = A.grids[e];
     uint32_t q = index;
     const int i_pz = q % G.n[4]; q /= G.n[4];
@@ -147,44 +143,52 @@ __device__ void eval_seed64(const BestArgs &A, int e, uint32_t index, Eval64 &ou
     const float *drift = A.drift_tab + (size_t)e * A.W;
     int n = 0, turn = 0, m = 0, n_match = 0, n_rec = 0;
     bool cn = true;
-    int cand[9];
     double a = A.kq / p, p_of_a = p;
     while (n < A.max_steps) {
         if (p != p_of_a) { a = A.kq / p; p_of_a = p; }                  // a = kappa q / p_n (C5/C6)
         double rn[3], Tn[3];
         rkn_step64(A.g, a, A.h, r, T, rn, Tn);
         if (cn) {
-            const int nc = candidates64(A.g, bits, r, cand);
-            for (int ic = 0; ic < nc; ++ic) {
-                const int w = cand[ic];
+            const int w = lane_candidate(A.g, s_layer, bits, r, lane);
+            bool matched = false;
+            double r2 = 0.0, ad = 0.0;
+            if (w >= 0) {
                 const float *wr = A.g.wire5 + (size_t)w * 5;
                 double d0[3], d1[3], tp;
                 wire_offset64(wr, r, d0, &tp);
                 const double g0 = d0[0] * T[0] + d0[1] * T[1] + d0[2] * T[2];
-                if (!(g0 <= 0.0)) continue;
                 wire_offset64(wr, rn, d1, &tp);
                 const double g1 = d1[0] * Tn[0] + d1[1] * Tn[1] + d1[2] * Tn[2];
-                if (!(g1 > 0.0)) continue;
-                const double tau = g0 / (g0 - g1);
-                double P[3], d[3];
+                if (g0 <= 0.0 && g1 > 0.0) {
+                    const double tau = g0 / (g0 - g1);
+                    double P[3], d[3];
 #pragma unroll
-                for (int i = 0; i < 3; ++i) P[i] = r[i] + tau * (rn[i] - r[i]);
-                wire_offset64(wr, P, d, &tp);
-                const double D = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-                const double zw = tp * (double)wr[4];
-                const double resid = D - (double)drift[w];
-                if (fabs(zw) <= A.g.z_half && resid * resid < A.lambda) {
-                    n_match += 1;
-                    chi2 += resid * resid;
-                    if (rec) {                      // matched approaches in path order, replayed by label_kernel
-                        if (n_rec < kRecCap) { rec[n_rec].wire = w; rec[n_rec].turn = turn; rec[n_rec].absd = fabs(resid); }
-                        n_rec += 1;
+                    for (int i = 0; i < 3; ++i) P[i] = r[i] + tau * (rn[i] - r[i]);
+                    wire_offset64(wr, P, d, &tp);
+                    const double D = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+                    const double zw = tp * (double)wr[4];
+                    const double resid = D - (double)__ldg(drift + w);
+                    r2 = resid * resid; ad = fabs(resid);
+                    matched = fabs(zw) <= A.g.z_half && r2 < A.lambda;
+                }
+            }
+            unsigned pend = __ballot_sync(full, matched);
+            while (pend) {                              // fold the matches in ascending wire id
+                const int wmin = __reduce_min_sync(full, (pend >> lane) & 1u ? w : 0x7fffffff);
+                const int src = __ffs(__ballot_sync(full, ((pend >> lane) & 1u) && w == wmin)) - 1;
+                const double r2s = __shfl_sync(full, r2, src), ads = __shfl_sync(full, ad, src);
+                n_match += 1;
+                chi2 += r2s;
+                if (lane == 0) {
+                    if (rec) {                          // matched approaches in path order, replayed by label_kernel
+                        if (n_rec < kRecCap) { rec[n_rec].wire = wmin; rec[n_rec].turn = turn; rec[n_rec].absd = ads; }
                     }
-                    if (wire_label) {               // C12: smallest |resid| wins, ties -> earliest
-                        const double ad = fabs(resid);
-                        if (wire_label[w] < 0 || ad < wire_best[w]) { wire_label[w] = turn; wire_best[w] = ad; }
+                    if (wire_label) {                   // C12: smallest |resid| wins, ties -> earliest
+                        if (wire_label[wmin] < 0 || ads < wire_best[wmin]) { wire_label[wmin] = turn; wire_best[wmin] = ads; }
                     }
                 }
+                n_rec += 1;
+                pend &= ~(1u << src);
             }
             m += 1;
         }
@@ -202,7 +206,13 @@ __device__ void eval_seed64(const BestArgs &A, int e, uint32_t index, Eval64 &ou
             break;
     }
     out.n_match = n_match; out.chi2 = chi2; out.n_steps = n; out.turns = turn; out.m_gas = m;
-    if (rec_count) *rec_count = n_rec;
+    if (rec_count && lane == 0) *rec_count = n_rec;
+}
+
+__device__ __forceinline__ void load_layers(const Geom64 &g, LayerDev *s_layer)
+{
+    for (int i = threadIdx.x; i < g.n_layers; i += blockDim.x) s_layer[i] = g.layers[i];
+    __syncthreads();
 }
 
 __device__ __forceinline__ uint32_t pool_size(const unsigned long long *counters, uint32_t cap)
@@ -217,26 +227,36 @@ __device__ __forceinline__ bool qualifies(const PoolEntry &pe, const uint64_t *b
     return pe.S32 >= Smax - margin;
 }
 
-// one thread per pool entry: fp64 score of the entries within the margin of the final fp32 maximum
-__global__ void rescore_kernel(const BestArgs A, const PoolEntry *pool, uint32_t pool_cap,
+// one warp per pool entry: fp64 score of the entries within the margin of the final fp32 maximum
+__global__ void __launch_bounds__(128) rescore_kernel(const BestArgs A, const PoolEntry *pool, uint32_t pool_cap,
                                const unsigned long long *counters, const uint64_t *best_key, float margin,
                                double *pool_S64, double *pool_chi2, int32_t *pool_nmatch,
                                unsigned long long *ev_maxS, ApproachRec *rec, int32_t *rec_count, int32_t *pool_slot,
                                int32_t *slot_counter)
 {
-    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    __shared__ LayerDev s_layer[CDC_MAX_LAYERS];
+    load_layers(A.g, s_layer);
+    const uint32_t i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
     if (i >= pool_size(counters, pool_cap)) return;
     const PoolEntry pe = pool[i];
-    if (!qualifies(pe, best_key, margin)) { pool_S64[i] = -1.0; pool_slot[i] = -1; return; }
+    if (!qualifies(pe, best_key, margin)) {
+        if (lane == 0) { pool_S64[i] = -1.0; pool_slot[i] = -1; }
+        return;
+    }
     Eval64 ev;
-    const int slot = atomicAdd(slot_counter, 1);
+    int slot = 0;
+    if (lane == 0) slot = atomicAdd(slot_counter, 1);
+    slot = __shfl_sync(0xffffffffu, slot, 0);
     const bool have = slot < kRecSlots;
-    pool_slot[i] = have ? slot : -1;
-    eval_seed64(A, (int)pe.event, pe.index, ev, nullptr, nullptr, have ? rec + (size_t)slot * kRecCap : nullptr,
+    eval_seed64(A, s_layer, (int)pe.event, pe.index, ev, nullptr, nullptr, have ? rec + (size_t)slot * kRecCap : nullptr,
                 have ? rec_count + slot : nullptr);
-    const double S = (double)ev.n_match - ev.chi2 / A.lambda;           // C10
-    pool_S64[i] = S; pool_chi2[i] = ev.chi2; pool_nmatch[i] = ev.n_match;
-    atomicMax(ev_maxS + pe.event, (unsigned long long)__double_as_longlong(S > 0.0 ? S : 0.0));
+    if (lane == 0) {
+        const double S = (double)ev.n_match - ev.chi2 / A.lambda;       // C10
+        pool_slot[i] = have ? slot : -1;
+        pool_S64[i] = S; pool_chi2[i] = ev.chi2; pool_nmatch[i] = ev.n_match;
+        atomicMax(ev_maxS + pe.event, (unsigned long long)__double_as_longlong(S > 0.0 ? S : 0.0));
+    }
 }
 
 // ties -> lowest linear index
@@ -272,15 +292,19 @@ __global__ void label_kernel(const BestArgs A, int n_events, const unsigned long
                              const double *pool_chi2, const int32_t *pool_nmatch, const int32_t *pool_slot,
                              const ApproachRec *rec, const int32_t *rec_count, const int32_t *ev_slot)
 {
-    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    __shared__ LayerDev s_layer[CDC_MAX_LAYERS];
+    load_layers(A.g, s_layer);
+    const int e = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;        // one warp per event
+    const int lane = threadIdx.x & 31;
     if (e >= n_events) return;
     const unsigned long long b = ev_best[e];
     if (b == ~0ull) {                      // no candidate survived (pool overflow): report "none"
-        best_seed[e] = -1; best_n_match[e] = 0; best_chi2[e] = 0.0;
+        if (lane == 0) { best_seed[e] = -1; best_n_match[e] = 0; best_chi2[e] = 0.0; }
         return;
     }
     const int slot = ev_slot[e];
     if (slot >= 0) {                       // replay the recorded matched approaches (path order) -- reading C12
+        if (lane != 0) return;
         int32_t *lab = wire_label + (size_t)e * A.W;
         double *bst = wire_best + (size_t)e * A.W;
         const ApproachRec *r = rec + (size_t)slot * kRecCap;
@@ -298,8 +322,8 @@ __global__ void label_kernel(const BestArgs A, int n_events, const unsigned long
         return;
     }
     Eval64 ev;                             // no usable record (slot table full or list overflow): propagate again
-    eval_seed64(A, e, (uint32_t)b, ev, wire_label + (size_t)e * A.W, wire_best + (size_t)e * A.W, nullptr, nullptr);
-    best_seed[e] = (int64_t)b; best_n_match[e] = (uint32_t)ev.n_match; best_chi2[e] = ev.chi2;
+    eval_seed64(A, s_layer, e, (uint32_t)b, ev, wire_label + (size_t)e * A.W, wire_best + (size_t)e * A.W, nullptr, nullptr);
+    if (lane == 0) { best_seed[e] = (int64_t)b; best_n_match[e] = (uint32_t)ev.n_match; best_chi2[e] = ev.chi2; }
 }
 
 __global__ void fill_i32(int32_t *p, size_t n, int32_t v)
@@ -332,7 +356,7 @@ cudaError_t launch_best_track(const BestLaunch &L, cudaStream_t s)
     if ((e = cudaMemsetAsync(L.d_ev_slot, 0xFF, sizeof(int32_t) * (size_t)L.n_events, s)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(L.d_slot_counter, 0, sizeof(int32_t), s)) != cudaSuccess) return e;
     const unsigned nb = (L.pool_cap + 63) / 64;
-    rescore_kernel<<<nb, 64, 0, s>>>(A, L.d_pool, L.pool_cap, L.d_counters, L.d_best_key, L.margin, L.d_pool_S64,
+    rescore_kernel<<<(L.pool_cap + 3) / 4, 128, 0, s>>>(A, L.d_pool, L.pool_cap, L.d_counters, L.d_best_key, L.margin, L.d_pool_S64,
                                      L.d_pool_chi2, L.d_pool_nmatch, L.d_ev_maxS, L.d_rec, L.d_rec_count, L.d_pool_slot,
                                      L.d_slot_counter);
     pick_kernel<<<nb, 64, 0, s>>>(L.d_pool, L.pool_cap, L.d_counters, L.d_pool_S64, L.d_ev_maxS, L.d_ev_best);
@@ -340,7 +364,7 @@ cudaError_t launch_best_track(const BestLaunch &L, cudaStream_t s)
                                   L.d_rec_count, L.d_ev_slot);
     const size_t nw = (size_t)L.n_events * L.W;
     fill_i32<<<(unsigned)((nw + 255) / 256), 256, 0, s>>>(L.d_wire_label, nw, -1);
-    label_kernel<<<(L.n_events + 31) / 32, 32, 0, s>>>(A, L.n_events, L.d_ev_best, L.d_wire_label, L.d_wire_best,
+    label_kernel<<<(L.n_events + 3) / 4, 128, 0, s>>>(A, L.n_events, L.d_ev_best, L.d_wire_label, L.d_wire_best,
                                                          L.d_best_seed, L.d_best_n_match, L.d_best_chi2, L.d_pool,
                                                          L.pool_cap, L.d_counters, L.d_pool_chi2, L.d_pool_nmatch,
                                                          L.d_pool_slot, L.d_rec, L.d_rec_count, L.d_ev_slot);
