@@ -32,6 +32,19 @@ FLOPS_LOOKUP, FLOPS_G, FLOPS_APPROACH = 43.0, 22.0, 35.0
 PEAK_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # 74.4: 148 SMs x 128 FP32 lanes x 2 x 1965 MHz (B200_PROFILING.md)
 
 
+def measured_traffic(workload):
+    """dram bytes per launch of the scan kernel from the committed ncu capture (profiles/), or None."""
+    try:
+        import csv
+        with open(os.path.join(ROOT, "profiles", "scan_kernel_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload and row["dram_bytes_read"]:
+                    return int(row["dram_bytes_read"]) + int(row["dram_bytes_write"] or 0)
+    except OSError:
+        pass
+    return None
+
+
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -236,7 +249,7 @@ def run_ours(args):
                 "e2e": {"value": seeds_all * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
                 "gpu_launches": int(launches),
                 "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s",
-                             "frac": achieved / PEAK_FP32_TFLOPS, "traffic": None, "kernel": "seed_scan_kernel",
+                             "frac": achieved / PEAK_FP32_TFLOPS, "traffic": measured_traffic(args.workload), "kernel": "seed_scan_kernel",
                              "flops_per_rkn_step": flops / max(acc["n_steps"], 1),
                              "peak_source": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (nominal, B200_PROFILING.md)"}}
         f, _ = B.cdc_fp32_peak_probe(4096)
