@@ -55,6 +55,9 @@ def parse():
     ap.add_argument("--events", type=int, default=0, help="events per GPU (0 = 1, or 16 for cfg3)")
     ap.add_argument("--grid-n", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true",
+                    help="BASELINE.json configs[4]: throughput of the scan over grid size, batch size and step size "
+                         "(one JSON line per point; not the driver's bench line)")
     return ap.parse_args()
 
 
@@ -265,6 +268,47 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """configs[4] as a star (DESIGN.md section 4): grid n in {8,12,16,24,32} at batch 1; batch in {1,...,1024} at 16^5;
+    h in {1,2,4} mm at 16^5 x 16 events (max_steps = 9000 mm / h).  Field, hits and noise of configs[3].  Beyond 64 events the
+    batch repeats the 64 generated ones (their hit tables are still uploaded and scanned separately)."""
+    import dataclasses
+    import torch
+    from paper_1908_01949_b200 import api, binding as B
+    torch.cuda.set_device(0)
+    cfg = synth.CONFIGS[4]
+    geom = synth.make_geometry(); field = synth.make_table_field()
+    base = synth.generate_events(cfg, geom, field, 64)
+    sc = api.SeedScanner(geom, field)
+    points = [("grid", n, 1, 2.0) for n in (8, 12, 16, 24, 32)] + \
+             [("batch", 16, b, 2.0) for b in (1, 4, 16, 64, 256, 1024)] + [("step", 16, 16, h) for h in (1.0, 2.0, 4.0)]
+    for axis, n, batch, h in points:
+        events = [base[i % len(base)] for i in range(batch)]
+        grids = [synth.truth_anchored_grid(ev.seed, n)[0] for ev in events]
+        off, w, d = synth.pack_hits(events)
+        specs = B.grid_specs(grids)
+        P = B.scan_params(h, int(round(9000.0 / h)), cfg.window_mm)
+        ev = B.Events(sc.geometry, off, w, d)
+        d_key = torch.zeros(batch, dtype=torch.int64, device="cuda")
+        ms = []
+        for it in range(3):
+            B.cdc_seed_scan(sc.geometry, ev, specs, P, d_key)
+            st = B.cdc_scan_get_stats(ev)
+            if it:
+                ms.append(st["kernel_ms"])
+        t = float(np.mean(ms)) * 1e-3
+        flops = FLOPS_STEP[1] * st["n_steps"] + FLOPS_LOOKUP * st["n_lookups"] + \
+            FLOPS_G * (st["n_approach_tests"] + st["n_g1"]) + FLOPS_APPROACH * st["n_approaches"]
+        print(json.dumps({"sweep_axis": axis, "grid_n": n, "events": batch, "h_mm": h, "seeds": st["n_seeds"],
+                          "rkn_steps": st["n_steps"], "kernel_ms": t * 1e3, "seeds_per_s": st["n_seeds"] / t,
+                          "rkn_steps_per_s": st["n_steps"] / t, "events_per_s": batch / t,
+                          "tflops": flops / t / 1e12, "frac_fp32_peak": flops / t / 1e12 / PEAK_FP32_TFLOPS}), flush=True)
+        ev.close()
+
+
 if __name__ == "__main__":
     a = parse()
-    run_reference(a) if a.impl == "reference" else run_ours(a)
+    if a.sweep:
+        run_sweep(a)
+    else:
+        run_reference(a) if a.impl == "reference" else run_ours(a)
