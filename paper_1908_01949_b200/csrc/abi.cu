@@ -33,7 +33,7 @@ cudaError_t dev_alloc(T **p, size_t n)
 void free_geometry(cdc_geometry *g)
 {
     if (!g) return;
-    cudaFree(g->d_wire4); cudaFree(g->d_wire5); cudaFree(g->d_field); cudaFree(g->d_layers);
+    cudaFree(g->d_wire4); cudaFree(g->d_wire5); cudaFree(g->d_field); cudaFree(g->d_cells); cudaFree(g->d_layers);
     delete g;
 }
 
@@ -171,6 +171,22 @@ extern "C" int32_t cdc_geometry_create(const cdc_geometry_desc *gd, const cdc_fi
     if (fd->kind == 1) {
         G_CUDA(dev_alloc(&g->d_field, (size_t)fd->nr * fd->nz));
         G_CUDA(cudaMemcpy(g->d_field, g->field_tab.data(), sizeof(float2) * (size_t)fd->nr * fd->nz, cudaMemcpyHostToDevice));
+        // per-cell bilinear coefficients for the fp32 scan: B(wr, wz) = c0 + c_r wr + c_z wz + c_rz wr wz
+        // (differences of the fp32 node values taken in fp64, rounded once)
+        const int ncr = fd->nr - 1, ncz = fd->nz - 1;
+        std::vector<float4> cells((size_t)ncr * ncz * 2);
+        for (int iz = 0; iz < ncz; ++iz)
+            for (int ir = 0; ir < ncr; ++ir)
+                for (int c = 0; c < 2; ++c) {
+                    const double n00 = g->field_tab[((size_t)iz * fd->nr + ir) * 2 + c];
+                    const double n01 = g->field_tab[((size_t)iz * fd->nr + ir + 1) * 2 + c];
+                    const double n10 = g->field_tab[((size_t)(iz + 1) * fd->nr + ir) * 2 + c];
+                    const double n11 = g->field_tab[((size_t)(iz + 1) * fd->nr + ir + 1) * 2 + c];
+                    cells[((size_t)iz * ncr + ir) * 2 + c] =
+                        make_float4((float)n00, (float)(n01 - n00), (float)(n10 - n00), (float)(n11 - n10 - n01 + n00));
+                }
+        G_CUDA(dev_alloc(&g->d_cells, cells.size()));
+        G_CUDA(cudaMemcpy(g->d_cells, cells.data(), sizeof(float4) * cells.size(), cudaMemcpyHostToDevice));
     }
 #undef G_CUDA
     GeomDev &d = g->gd;
@@ -184,7 +200,8 @@ extern "C" int32_t cdc_geometry_create(const cdc_geometry_desc *gd, const cdc_fi
     f.kind = fd->kind; f.bz = (float)fd->bz_T; f.nr = fd->nr; f.nz = fd->nz;
     f.r0 = (float)fd->r0_mm; f.z0 = (float)fd->z0_mm;
     f.inv_dr = fd->kind == 1 ? (float)(1.0 / fd->dr_mm) : 0.f; f.inv_dz = fd->kind == 1 ? (float)(1.0 / fd->dz_mm) : 0.f;
-    f.tab = g->d_field;
+    f.tab = g->d_field; f.cells = g->d_cells;
+    f.cr = fd->kind == 1 ? (float)(-fd->r0_mm / fd->dr_mm) : 0.f; f.cz = fd->kind == 1 ? (float)(-fd->z0_mm / fd->dz_mm) : 0.f;
     Geom64 &q = g->g64;
     q.n_layers = L; q.n_wires_total = g->W; q.R0 = g->R0; q.z_half = g->z_half; q.r_out = g->r_out;
     q.wire5 = g->d_wire5; q.layers = g->d_layers; q.r_first = d.r_first; q.inv_pitch = d.inv_pitch; q.tan_abs = d.tan_abs;

@@ -30,7 +30,9 @@ struct FieldDev {
     float bz;                // uniform field
     int32_t nr, nz;
     float r0, z0, inv_dr, inv_dz;
-    const float2 *tab;       // [nz][nr] (B_r, B_z)
+    float cr, cz;            // -r0 / dr, -z0 / dz: cell coordinate = fma(rho, inv_dr, cr)
+    const float2 *tab;       // [nz][nr] (B_r, B_z) nodes (fp64 path)
+    const float4 *cells;     // [nz-1][nr-1][2]: bilinear coefficients (c0, c_r, c_z, c_rz) of B_r, then of B_z
 };
 
 struct GeomDev {
@@ -72,6 +74,7 @@ struct cdc_geometry {
     float4 *d_wire4 = nullptr;
     float *d_wire5 = nullptr;
     float2 *d_field = nullptr;
+    float4 *d_cells = nullptr;
     LayerDev *d_layers = nullptr;
     GeomDev gd{};
     FieldDev fd{};

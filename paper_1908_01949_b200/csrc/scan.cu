@@ -73,21 +73,20 @@ __device__ __forceinline__ void field_at(const FieldDev &F, float x, float y, fl
     if (FIELD == 0) {
         Bx = 0.0f; By = 0.0f; Bz = F.bz;
     } else {
-        float rho2 = fmaf(x, x, y * y);
-        float inv_rho = rho2 > 0.0f ? rsqrtf(rho2) : 0.0f;
-        float rho = rho2 * inv_rho;
-        float fr = (rho - F.r0) * F.inv_dr;
-        float fz = (z - F.z0) * F.inv_dz;
-        int ir = min(max(__float2int_rd(fr), 0), F.nr - 2);
-        int iz = min(max(__float2int_rd(fz), 0), F.nz - 2);
-        float wr = fr - (float)ir, wz = fz - (float)iz;
-        const float2 *p = F.tab + iz * F.nr + ir;
-        float2 n00 = __ldg(p), n01 = __ldg(p + 1), n10 = __ldg(p + F.nr), n11 = __ldg(p + F.nr + 1);
-        float br0 = fmaf(wr, n01.x - n00.x, n00.x), br1 = fmaf(wr, n11.x - n10.x, n10.x);
-        float bz0 = fmaf(wr, n01.y - n00.y, n00.y), bz1 = fmaf(wr, n11.y - n10.y, n10.y);
-        float Br = fmaf(wz, br1 - br0, br0);
-        Bz = fmaf(wz, bz1 - bz0, bz0);
-        float s = Br * inv_rho;
+        // validated at create time: the table covers every point a live track or its stages can reach, so the
+        // cell index needs no lower clamp; the unsigned min only keeps a non-finite state inside the allocation
+        const float rho2 = fmaf(x, x, y * y);
+        const float inv_rho = rsqrtf(fmaxf(rho2, 1e-30f));
+        const float rho = rho2 * inv_rho;
+        const float fr = fmaf(rho, F.inv_dr, F.cr), fz = fmaf(z, F.inv_dz, F.cz);
+        const unsigned ir = min((unsigned)__float2int_rd(fr), (unsigned)(F.nr - 2));
+        const unsigned iz = min((unsigned)__float2int_rd(fz), (unsigned)(F.nz - 2));
+        const float wr = fr - (float)ir, wz = fz - (float)iz;
+        const float4 *c = F.cells + 2u * (iz * (unsigned)(F.nr - 1) + ir);
+        const float4 cr = __ldg(c), cz = __ldg(c + 1);
+        const float Br = fmaf(wz, fmaf(wr, cr.w, cr.z), fmaf(wr, cr.y, cr.x));
+        Bz = fmaf(wz, fmaf(wr, cz.w, cz.z), fmaf(wr, cz.y, cz.x));
+        const float s = Br * inv_rho;
         Bx = s * x; By = s * y;
     }
 }
