@@ -220,16 +220,18 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
     __syncthreads();
     const float *drift_e = A.drift_tab + (size_t)e * A.gd.n_wires_total;
 
-    // ---- A3: thread -> seed.  theta is the lane-fastest axis, then px, py, z, pz: neighbouring lanes then
-    // share (z0, p) and leave the chamber within a few steps of one another.
+    // ---- A3: thread -> seed.  z0 is the lane-fastest axis, then theta, px, py, pz.  Seeds that differ only in z0 have
+    // the same (x, y) path up to the field's z dependence, so the 32 tracks of a warp pass the same wires within a
+    // step or two of one another: lookups, live-wire slots and approach code run with most lanes active.  They leave
+    // the chamber a few tens of steps apart (the z0 pitch over T_z h), a ~4 % tail.
     const int t = blockIdx.x * kBlock + threadIdx.x;
     const bool valid = t < G.n_seeds;
     int q = valid ? t : 0;
+    const int i_z = q % G.n[1]; q /= G.n[1];
     const int i_th = q % G.n[0]; q /= G.n[0];
     const int i_px = q % G.n[2]; q /= G.n[2];
-    const int i_py = q % G.n[3]; q /= G.n[3];
-    const int i_z = q % G.n[1];
-    const int i_pz = q / G.n[1];
+    const int i_py = q % G.n[3];
+    const int i_pz = q / G.n[3];
     const uint32_t index = (uint32_t)((((i_th * G.n[1] + i_z) * G.n[2] + i_px) * G.n[3] + i_py) * G.n[4] + i_pz);
 
     float xh, xl, yh, yl, zh, zl, Txh, Txl, Tyh, Tyl, Tzh, Tzl, a, epsT, p0h, p0l;
