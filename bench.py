@@ -27,7 +27,7 @@ from paper_1908_01949_b200 import synth  # noqa: E402
 METRIC = "seed_propagations_per_s"
 UNIT = "seeds/s"
 # Algorithmic FP32 flops (FMA = 2) of the scan kernel's arithmetic, DESIGN.md section 7
-FLOPS_STEP = {0: 78.0, 1: 255.0}        # per RKN step, uniform / tabulated field (compensated state included)
+FLOPS_STEP = {0: 78.0, 1: 237.0}        # per RKN step, uniform / tabulated field (compensated state included)
 FLOPS_LOOKUP, FLOPS_G, FLOPS_APPROACH = 43.0, 22.0, 35.0
 PEAK_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # 74.4: 148 SMs x 128 FP32 lanes x 2 x 1965 MHz (B200_PROFILING.md)
 
@@ -48,7 +48,7 @@ def measured_traffic(workload):
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg1", choices=["cfg0", "cfg1", "cfg2", "cfg3"])
@@ -74,17 +74,19 @@ def make_workload(args, rank):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
-    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe).  The sampler
+    runs from before the warm-up; only the samples stamped inside [mark_start, mark_stop] are reported (if the region
+    is shorter than the sampling period, the sample nearest to it, flagged with "samples": 0)."""
+    Q = "timestamp,clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
 
     def __init__(self, index):
-        self.rows, self.proc, self.index = [], None, index
+        self.rows, self.proc, self.index, self.t0, self.t1 = [], None, index, None, None
 
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             threading.Thread(target=self._read, daemon=True).start()
         except OSError:
@@ -92,21 +94,34 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([x.strip() for x in line.split(",")])
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def mark_start(self):
+        self.t0 = time.time()
+
+    def mark_stop(self):
+        self.t1 = time.time()
 
     def stop(self):
         if self.proc:
+            time.sleep(0.12)                       # let the sample that covers the end of the region arrive
             self.proc.terminate()
             try:
                 self.proc.wait(timeout=2)
             except Exception:
                 pass
-        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
-        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        ok = [(t, r) for t, r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        inside = [r for t, r in ok if self.t0 is not None and self.t0 <= t <= self.t1 + 0.06]
+        n_inside = len(inside)
+        if not inside and ok:
+            mid = 0.5 * ((self.t0 or 0) + (self.t1 or 0))
+            inside = [min(ok, key=lambda tr: abs(tr[0] - mid))[1]]
+        sm = [float(r[1]) for r in inside]
+        mx = [float(r[2]) for r in inside]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = sorted({names[i] for r in self.rows if len(r) >= 6 for i in range(4) if r[2 + i].lower() == "active"})
+        reasons = sorted({names[i] for r in inside for i in range(4) if r[3 + i].lower() == "active"})
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": reasons, "samples": len(sm)}
+                "reasons": reasons, "samples": n_inside}
 
 
 def oracle_sample_time(cfg, geom, field, ev, grid, n_sample, key):
@@ -190,10 +205,11 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    sampler = ClockSampler(local); sampler.start()
     for _ in range(args.warmup):
         flush.fill_(1); step().close()
     barrier()
-    sampler = ClockSampler(local); sampler.start()
+    sampler.mark_start()
     l0 = B.cdc_kernel_launch_count()
     ms, kernel_ms, acc = [], [], {}
     for _ in range(args.steps):
@@ -207,6 +223,7 @@ def run_ours(args):
             acc[k] = acc.get(k, 0) + v
         ev.close()
     barrier()
+    sampler.mark_stop()
     launches = B.cdc_kernel_launch_count() - l0
     clocks = sampler.stop()
     best = (d_seed.cpu().numpy().tolist(), d_nm.cpu().numpy().tolist())
