@@ -184,6 +184,24 @@ int32_t cdc_find_tracks_host(const cdc_geometry *g, int32_t n_events, const int3
                              double *h_best_chi2, uint64_t *h_best_key, int32_t *h_labels,
                              double *h_ranges_or_null, void *stream);
 
+/* Coarse-to-fine refinement around the seed scan ("we took the several candidate seeds with the lowest
+ * E, and make other seed sets around them with finer granularity ... repeated ten times"; reading C17):
+ * iteration 0 scans h_grids; iteration t = 1..n_iterations scans the 3^5 nodes q_parent + {-d, 0, +d}^5, d = 2^(T-t),
+ * around each of the n_parents best seeds so far, on the integer lattice of the finest pitch step / 2^T
+ * (value = lo + q * step / 2^T); parents are ordered by (S descending, sub-grid rank, index), duplicates skipped.
+ * Outputs (host, per event): best seed values [E][5], S, n_match, chi2, lattice point q [E][5]; labels per hit
+ * (optional); the parents of every iteration (optional): S [E][T+1][K] (-1 = none) and q [E][T+1][K][5].
+ * Scores, selection and labels are fp64 (bit-equal to a plain IEEE evaluation).  Synchronises. */
+typedef struct {
+    int32_t n_parents;        /* K, 1..8 */
+    int32_t n_iterations;     /* T, 0..20 (the paper: ten) */
+} cdc_refine_params;
+int32_t cdc_refine_tracks(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec *h_grids,
+                          const cdc_scan_params *params, const cdc_refine_params *rp, double *h_best_seed,
+                          double *h_best_S, uint32_t *h_best_n_match, double *h_best_chi2, int64_t *h_best_q,
+                          int32_t *h_labels_or_null, double *h_trace_S_or_null, int64_t *h_trace_q_or_null,
+                          void *stream);
+
 /* Number of kernels this library has launched in this process so far (bench.py's gpu_launches). */
 uint64_t cdc_kernel_launch_count(void);
 

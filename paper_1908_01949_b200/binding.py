@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(HERE, "libcdc_seedscan.so")
 EXPORTS = ["cdc_last_error", "cdc_geometry_create", "cdc_geometry_destroy", "cdc_geometry_wire_table",
            "cdc_event_upload", "cdc_events_destroy", "cdc_events_tables", "cdc_hough_dims",
            "cdc_hough_seed_ranges", "cdc_seed_scan", "cdc_scan_get_stats", "cdc_best_track",
-           "cdc_find_tracks_host", "cdc_fp32_peak_probe", "cdc_kernel_launch_count"]
+           "cdc_find_tracks_host", "cdc_refine_tracks", "cdc_fp32_peak_probe", "cdc_kernel_launch_count"]
 
 
 class CdcError(RuntimeError):
@@ -51,6 +51,10 @@ class ScanParams(C.Structure):
 class HoughParams(C.Structure):
     _fields_ = [(k, C.c_double) for k in ("bin_xy_mm", "bin_R_mm", "tol_mm", "R_lo_mm", "R_hi_mm", "half_xy_mm",
                                           "origin_mm", "half_theta_rad", "half_pt_MeV")]
+
+
+class RefineParams(C.Structure):
+    _fields_ = [("n_parents", C.c_int32), ("n_iterations", C.c_int32)]
 
 
 class ScanStats(C.Structure):
@@ -248,6 +252,22 @@ def cdc_find_tracks_host(geometry: Geometry, hit_offsets, wire_id, drift_mm, gri
                                       _hp(key), _hp(lab), _hp(ranges), _stream(stream)))
     return dict(best_seed=seed, best_n_match=nm, best_chi2=chi2, best_key=key, labels=lab[:int(off[-1])],
                 ranges=ranges)
+
+
+def cdc_refine_tracks(geometry: Geometry, events: Events, grids: C.Array, params: ScanParams, n_parents: int = 8,
+                      n_iterations: int = 10, want_labels: bool = True, want_trace: bool = True, stream=None) -> dict:
+    """Coarse-to-fine refinement.  Host (numpy) outputs."""
+    E, K, T = events.n_events, int(n_parents), int(n_iterations)
+    seed = np.zeros((E, 5)); S = np.zeros(E); nm = np.zeros(E, dtype=np.uint32); chi2 = np.zeros(E)
+    q = np.zeros((E, 5), dtype=np.int64)
+    lab = np.zeros(max(events.n_hits, 1), dtype=np.int32) if want_labels else None
+    tS = np.zeros((E, T + 1, K)) if want_trace else None
+    tq = np.zeros((E, T + 1, K, 5), dtype=np.int64) if want_trace else None
+    rp = RefineParams(K, T)
+    _check(lib().cdc_refine_tracks(geometry.handle, events.handle, grids, C.byref(params), C.byref(rp), _hp(seed), _hp(S),
+                                   _hp(nm), _hp(chi2), _hp(q), _hp(lab), _hp(tS), _hp(tq), _stream(stream)))
+    return dict(seed=seed, S=S, n_match=nm, chi2=chi2, q=q, labels=None if lab is None else lab[:events.n_hits],
+                trace_S=tS, trace_q=tq)
 
 
 def cdc_kernel_launch_count() -> int:
