@@ -76,20 +76,22 @@ def test_truth_node_stays_first_parent_on_a_smear_free_event():
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("cfg_id,n0,K,T", [(0, 5, 4, 6), (1, 4, 8, 10)])
+@pytest.mark.parametrize("cfg_id,n0,K,T", [(0, 5, 4, 6), (1, 4, 8, 10), (2, 3, 3, 4), (3, 4, 2, 5)])
 def test_gpu_refinement_equals_oracle(cfg_id, n0, K, T):
+    """uniform field, noise, energy loss (cfg2) and tabulated field (cfg3)"""
     from paper_1908_01949_b200 import api, binding as B
     cfg = synth.CONFIGS[cfg_id]
-    geom = synth.make_geometry(); field = synth.make_uniform_field()
+    geom = synth.make_geometry()
+    field = synth.make_uniform_field() if cfg.field_kind == 0 else synth.make_table_field()
     events = synth.generate_events(cfg, geom, field, 2)
     shift = np.array([0.3, 0.4, -0.35, 0.25, 0.45]) * synth.HALF_WIDTH / 2
     grids = [synth.truth_anchored_grid(ev.seed + shift, n0)[0] for ev in events]
     sc = api.SeedScanner(geom, field)
     off, w, d = synth.pack_hits(events)
     E = sc.upload(off, w, d)
-    P = B.scan_params(cfg.h_mm, cfg.max_steps, cfg.window_mm)
+    P = B.scan_params(cfg.h_mm, cfg.max_steps, cfg.window_mm, cfg.eloss_MeV_per_mm)
     out = B.cdc_refine_tracks(sc.geometry, E, B.grid_specs(grids), P, n_parents=K, n_iterations=T)
-    params = dict(h=cfg.h_mm, max_steps=cfg.max_steps, window=cfg.window_mm)
+    params = dict(h=cfg.h_mm, max_steps=cfg.max_steps, window=cfg.window_mm, eloss=cfg.eloss_MeV_per_mm)
     for e, (ev, g0) in enumerate(zip(events, grids)):
         r = R.refine(geom, field, params, ev.wire_id, ev.drift_mm, g0, K=K, T=T)
         for t in range(T + 1):
