@@ -202,6 +202,17 @@ int32_t cdc_refine_tracks(const cdc_geometry *g, cdc_events *ev, const cdc_grid_
                           int32_t *h_labels_or_null, double *h_trace_S_or_null, int64_t *h_trace_q_or_null,
                           void *stream);
 
+/* Classification efficiency and purity per turn partition (Eq. (2), (3)) of hit -> turn labels against
+ * truth labels (-1 = noise), per event of `ev` (hits in upload order): d_confusion [E][n][n] (truth i classified as j),
+ * d_c_true [E][n], d_noise_into [E][n] (noise hits classified into a partition; not part of Eq. (3)'s sum),
+ * d_efficiency, d_purity [E][n] f64 (-1 where the denominator is 0).  n_turns <= 8.  Asynchronous. */
+int32_t cdc_classification_quality(const cdc_events *ev, int32_t n_turns, const int32_t *d_labels,
+                                   const int32_t *d_truth_turn, int32_t *d_confusion, int32_t *d_c_true,
+                                   int32_t *d_noise_into, double *d_efficiency, double *d_purity, void *stream);
+/* N_c: hits labelled (>= 0) by both of two independent scans, per event.  Asynchronous. */
+int32_t cdc_common_hits(const cdc_events *ev, const int32_t *d_labels_a, const int32_t *d_labels_b,
+                        int32_t *d_n_common, void *stream);
+
 /* Number of kernels this library has launched in this process so far (bench.py's gpu_launches). */
 uint64_t cdc_kernel_launch_count(void);
 

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(HERE, "libcdc_seedscan.so")
 EXPORTS = ["cdc_last_error", "cdc_geometry_create", "cdc_geometry_destroy", "cdc_geometry_wire_table",
            "cdc_event_upload", "cdc_events_destroy", "cdc_events_tables", "cdc_hough_dims",
            "cdc_hough_seed_ranges", "cdc_seed_scan", "cdc_scan_get_stats", "cdc_best_track",
-           "cdc_find_tracks_host", "cdc_refine_tracks", "cdc_fp32_peak_probe", "cdc_kernel_launch_count"]
+           "cdc_find_tracks_host", "cdc_refine_tracks", "cdc_classification_quality", "cdc_common_hits", "cdc_fp32_peak_probe", "cdc_kernel_launch_count"]
 
 
 class CdcError(RuntimeError):
@@ -268,6 +268,28 @@ def cdc_refine_tracks(geometry: Geometry, events: Events, grids: C.Array, params
                                    _hp(nm), _hp(chi2), _hp(q), _hp(lab), _hp(tS), _hp(tq), _stream(stream)))
     return dict(seed=seed, S=S, n_match=nm, chi2=chi2, q=q, labels=None if lab is None else lab[:events.n_hits],
                 trace_S=tS, trace_q=tq)
+
+
+def cdc_classification_quality(events: Events, n_turns: int, d_labels, d_truth, stream=None) -> dict:
+    """Eq. (2), (3) of the paper per event and turn partition; returns numpy arrays."""
+    import torch
+    E, n = events.n_events, int(n_turns)
+    conf = torch.zeros((E, n, n), dtype=torch.int32, device="cuda"); ct = torch.zeros((E, n), dtype=torch.int32, device="cuda")
+    ni = torch.zeros((E, n), dtype=torch.int32, device="cuda")
+    eff = torch.zeros((E, n), dtype=torch.float64, device="cuda"); pur = torch.zeros((E, n), dtype=torch.float64, device="cuda")
+    _check(lib().cdc_classification_quality(events.handle, C.c_int32(n), _dp(d_labels), _dp(d_truth), _dp(conf), _dp(ct),
+                                            _dp(ni), _dp(eff), _dp(pur), _stream(stream)))
+    torch.cuda.synchronize()
+    return dict(confusion=conf.cpu().numpy(), c_true=ct.cpu().numpy(), noise_into=ni.cpu().numpy(),
+                efficiency=eff.cpu().numpy(), purity=pur.cpu().numpy())
+
+
+def cdc_common_hits(events: Events, d_labels_a, d_labels_b, stream=None) -> np.ndarray:
+    import torch
+    out = torch.zeros(events.n_events, dtype=torch.int32, device="cuda")
+    _check(lib().cdc_common_hits(events.handle, _dp(d_labels_a), _dp(d_labels_b), _dp(out), _stream(stream)))
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
 
 
 def cdc_kernel_launch_count() -> int:

@@ -14,7 +14,7 @@ COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC,-ffp-contract=o
 SOURCES = {                      # file -> extra flags
     "abi.cu": [], "abi_events.cu": [], "abi_scan.cu": [], "abi_e2e.cu": [],
     "events.cu": [], "hough.cu": [], "scan.cu": ["-Xptxas", "-v"], "peak.cu": [],
-    "best.cu": ["-fmad=false"], "refine.cu": ["-fmad=false"], "abi_refine.cu": [],
+    "best.cu": ["-fmad=false"], "refine.cu": ["-fmad=false"], "abi_refine.cu": [], "quality.cu": [],
 }
 HEADERS = [os.path.join(CSRC, "cdc_internal.cuh"), os.path.join(CSRC, "eval64.cuh"), os.path.join(HERE, "..", "include", "cdc_seedscan.h")]
 
