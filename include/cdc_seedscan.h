@@ -209,9 +209,11 @@ int32_t cdc_refine_tracks(const cdc_geometry *g, cdc_events *ev, const cdc_grid_
 int32_t cdc_classification_quality(const cdc_events *ev, int32_t n_turns, const int32_t *d_labels,
                                    const int32_t *d_truth_turn, int32_t *d_confusion, int32_t *d_c_true,
                                    int32_t *d_noise_into, double *d_efficiency, double *d_purity, void *stream);
-/* N_c: hits labelled (>= 0) by both of two independent scans, per event.  Asynchronous. */
+/* N_c ("the number of hits commonly found from the both direction"): hits that scan A labels turn_a and
+ * scan B labels turn_b (a turn of -1 = any turn >= 0), per event.  A backward scan is an ordinary cdc_seed_scan with
+ * params->charge = -q and a grid around the exit-side seed with the momentum reversed.  Asynchronous. */
 int32_t cdc_common_hits(const cdc_events *ev, const int32_t *d_labels_a, const int32_t *d_labels_b,
-                        int32_t *d_n_common, void *stream);
+                        int32_t turn_a, int32_t turn_b, int32_t *d_n_common, void *stream);
 
 /* Number of kernels this library has launched in this process so far (bench.py's gpu_launches). */
 uint64_t cdc_kernel_launch_count(void);

@@ -32,9 +32,11 @@ def classification_quality(labels, truth, n_turns):
                 noise_into=np.array(noise_into, dtype=np.int32), efficiency=np.array(eff), purity=np.array(pur))
 
 
-def common_hits(labels_a, labels_b):
+def common_hits(labels_a, labels_b, turn_a=-1, turn_b=-1):
+    """hits that scan A labels turn_a and scan B labels turn_b (-1 = any turn >= 0)"""
     n = 0
     for a, b in zip(labels_a, labels_b):
-        if int(a) >= 0 and int(b) >= 0:
+        a, b = int(a), int(b)
+        if (a >= 0 if turn_a < 0 else a == turn_a) and (b >= 0 if turn_b < 0 else b == turn_b):
             n += 1
     return n

@@ -284,10 +284,11 @@ def cdc_classification_quality(events: Events, n_turns: int, d_labels, d_truth, 
                 efficiency=eff.cpu().numpy(), purity=pur.cpu().numpy())
 
 
-def cdc_common_hits(events: Events, d_labels_a, d_labels_b, stream=None) -> np.ndarray:
+def cdc_common_hits(events: Events, d_labels_a, d_labels_b, turn_a: int = -1, turn_b: int = -1, stream=None) -> np.ndarray:
     import torch
     out = torch.zeros(events.n_events, dtype=torch.int32, device="cuda")
-    _check(lib().cdc_common_hits(events.handle, _dp(d_labels_a), _dp(d_labels_b), _dp(out), _stream(stream)))
+    _check(lib().cdc_common_hits(events.handle, _dp(d_labels_a), _dp(d_labels_b), C.c_int32(turn_a), C.c_int32(turn_b),
+                                 _dp(out), _stream(stream)))
     torch.cuda.synchronize()
     return out.cpu().numpy()
 

@@ -39,11 +39,12 @@ __global__ void __launch_bounds__(256) quality_kernel(int n_turns, const int32_t
     }
 }
 
-__global__ void __launch_bounds__(256) common_kernel(const int32_t *offsets, const int32_t *la, const int32_t *lb, int32_t *n_common)
+__global__ void __launch_bounds__(256) common_kernel(const int32_t *offsets, const int32_t *la, const int32_t *lb, int ta, int tb,
+                                                     int32_t *n_common)
 {
     const int e = blockIdx.x;
     int c = 0;
-    for (int i = offsets[e] + threadIdx.x; i < offsets[e + 1]; i += blockDim.x) c += (la[i] >= 0 && lb[i] >= 0) ? 1 : 0;
+    for (int i = offsets[e] + threadIdx.x; i < offsets[e + 1]; i += blockDim.x) c += ((ta < 0 ? la[i] >= 0 : la[i] == ta) && (tb < 0 ? lb[i] >= 0 : lb[i] == tb)) ? 1 : 0;
     c = __reduce_add_sync(0xffffffffu, c);
     __shared__ int s[8];
     if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = c;
@@ -72,10 +73,10 @@ extern "C" int32_t cdc_classification_quality(const cdc_events *ev, int32_t n_tu
 }
 
 extern "C" int32_t cdc_common_hits(const cdc_events *ev, const int32_t *d_labels_a, const int32_t *d_labels_b,
-                                   int32_t *d_n_common, void *stream)
+                                   int32_t turn_a, int32_t turn_b, int32_t *d_n_common, void *stream)
 {
     if (!ev || !d_labels_a || !d_labels_b || !d_n_common) CDC_FAIL(CDC_ERR_INVALID, "cdc_common_hits: null argument");
-    common_kernel<<<ev->n_events, 256, 0, (cudaStream_t)stream>>>(ev->d_offsets, d_labels_a, d_labels_b, d_n_common);
+    common_kernel<<<ev->n_events, 256, 0, (cudaStream_t)stream>>>(ev->d_offsets, d_labels_a, d_labels_b, turn_a, turn_b, d_n_common);
     cdc_count_launch();
     CDC_CUDA(cudaGetLastError());
     return CDC_OK;

@@ -283,15 +283,20 @@ def find_crossings(geom: Geometry, field: Field, sim: Dict[str, np.ndarray],
 
 
 def truth_seed(geom: Geometry, field: Field, sim: Dict[str, np.ndarray], t: int,
-               charge: int = -1) -> Optional[Tuple[np.ndarray, float]]:
-    """State at the first outward crossing of rho = R0 of track t:
-    (theta, z, px, py, pz) and the path length at which it happens."""
+               charge: int = -1, inward: bool = False) -> Optional[Tuple[np.ndarray, float]]:
+    """State at the first outward crossing of rho = R0 of track t (the CDC entrance):
+    (theta, z, px, py, pz) and the path length at which it happens.  inward=True: the first inward crossing
+    after it (the CDC exit of the first turn partition), momentum as the particle has it there."""
     pos, tan, pp, alive, ds = sim["pos"][:, t], sim["tan"][:, t], sim["p"][:, t], sim["alive"][:, t], sim["ds"]
     rho2 = pos[:, 0] ** 2 + pos[:, 1] ** 2
     R0sq = geom.R0_mm ** 2
     idx = np.nonzero((rho2[:-1] < R0sq) & (rho2[1:] >= R0sq) & alive[1:])[0]
     if idx.size == 0:
         return None
+    if inward:
+        idx = np.nonzero((rho2[:-1] >= R0sq) & (rho2[1:] < R0sq) & alive[1:] & (np.arange(rho2.size - 1) > int(idx[0])))[0]
+        if idx.size == 0:
+            return None
     i = int(idx[0])
     r0, T0 = pos[i:i + 1], tan[i:i + 1]
     K = ((KAPPA * charge) / pp[i]) * np.cross(T0, _truth_field(field, r0))
@@ -360,6 +365,8 @@ class Event:
     seed: np.ndarray          # (5,) f64, fp32-representable truth seed at R0
     n_turns: int
     n_signal: int
+    seed_exit: Optional[np.ndarray] = None   # (5,) f64: exit of the first turn partition with the momentum REVERSED
+                                             # (a backward scan starts here with the opposite charge), or None
 
 
 def _stream(seed: int, purpose: int) -> np.random.Generator:
@@ -424,6 +431,7 @@ def generate_events(cfg: EventConfig, geom: Geometry, field: Field, n_events: Op
                 if ts is None:
                     continue
                 seed, s_seed = ts
+                tx = truth_seed(geom, field, sim, loc, charge=charge, inward=True)
                 cr = cross[loc]
                 cr = cr[(cr["s"] <= s_seed + cfg.path_mm) & (cr["doca"] < cfg.drift_max_mm)]
                 _, first = np.unique(cr["wire"], return_index=True)     # one hit per wire, first wins
@@ -432,13 +440,13 @@ def generate_events(cfg: EventConfig, geom: Geometry, field: Field, n_events: Op
                 if int((counts >= 10).sum()) != want[pending[pe]] or \
                         int((counts >= 10).sum()) != int((counts > 0).sum()):
                     continue
-                accepted[pe] = (seed, cr)
+                accepted[pe] = (seed, cr, None if tx is None else tx[0])
         still = []
         for pe, e in enumerate(pending):
             if pe not in accepted:
                 still.append(e)
                 continue
-            seed, cr = accepted[pe]
+            seed, cr, seed_x = accepted[pe]
             sm = _stream(seeds[e], 1)
             g = _box_muller(sm.random(cr.shape[0]), sm.random(cr.shape[0]))
             drift = np.abs(cr["doca"] + sigma * g)
@@ -458,7 +466,8 @@ def generate_events(cfg: EventConfig, geom: Geometry, field: Field, n_events: Op
             o = np.argsort(w, kind="stable")
             done[e] = Event(wire_id=w[o].astype(np.int32), drift_mm=d[o].astype(np.float32),
                             truth_turn=t[o].astype(np.int32), seed=seed, n_turns=want[e],
-                            n_signal=int(sig_w.size))
+                            n_signal=int(sig_w.size),
+                            seed_exit=None if seed_x is None else seed_x * np.array([1.0, 1.0, -1.0, -1.0, -1.0]))
         pending = still
     return done  # type: ignore[return-value]
 
