@@ -65,6 +65,7 @@ extern "C" int32_t cdc_refine_tracks(const cdc_geometry *g, cdc_events *ev, cons
     L.d_drift_tab = ev->d_drift_tab; L.d_bits = ev->d_bits; L.d_offsets = ev->d_offsets; L.d_wire_id = ev->d_wire_id;
     L.W = ev->W; L.n_bit_words = ev->n_bit_words; L.max_hits_per_event = ev->max_hits_per_event;
     L.h = p->h_mm; L.window = p->window_mm; L.eloss = p->eloss_MeV_per_mm; L.max_steps = p->max_steps; L.charge = p->charge;
+    L.lookup_every64 = cdc_lookup_every64(g, p->h_mm, p->window_mm);
     L.d_wire_label = ev->d_wire_label; L.d_wire_best = ev->d_wire_best;
     CDC_CUDA(D.get(&L.d_cand_idx, (size_t)E * L.cap)); CDC_CUDA(D.get(&L.d_count, (size_t)E));
     CDC_CUDA(D.get(&L.d_S64, (size_t)E * L.cap)); CDC_CUDA(D.get(&L.d_chi2_64, (size_t)E * L.cap));

@@ -114,6 +114,15 @@ int32_t prepare_grids(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec
 
 }  // namespace
 
+int32_t cdc_lookup_every64(const cdc_geometry *g, double h_mm, double window_mm)
+{
+    const double dmax = 8.0 + window_mm + 0.05;
+    const double reach = sqrt(dmax * dmax + h_mm * h_mm) + 0.1;
+    const double excl3 = 1.5 * (g->excl + 0.2) - 0.3;           // 1.5 layer pitches / 1.5 cells (g->excl is one of them)
+    if (reach > excl3) return 1;
+    return std::max(1, std::min(1 + (int)floor((excl3 - reach) / h_mm), 16));
+}
+
 // ------------------------------------------------------------------------------------------------ A2
 extern "C" int32_t cdc_hough_dims(const cdc_hough_params *hp, int32_t *dims3)
 {
@@ -238,6 +247,7 @@ extern "C" int32_t cdc_best_track(const cdc_geometry *g, cdc_events *ev, const c
     L.d_offsets = ev->d_offsets; L.d_wire_id = ev->d_wire_id; L.d_drift = ev->d_drift; L.d_drift_tab = ev->d_drift_tab;
     L.d_bits = ev->d_bits; L.W = ev->W; L.n_bit_words = ev->n_bit_words; L.max_hits_per_event = ev->max_hits_per_event;
     L.h = p->h_mm; L.window = p->window_mm; L.eloss = p->eloss_MeV_per_mm; L.max_steps = p->max_steps; L.charge = p->charge;
+    L.lookup_every64 = cdc_lookup_every64(g, p->h_mm, p->window_mm);
     L.margin = (float)(p->rescore_margin > 0.0 ? p->rescore_margin : kDefaultMargin);
     L.d_best_key = d_best_key; L.d_pool = ev->d_pool; L.pool_cap = ev->pool_cap; L.d_counters = ev->d_counters;
     L.d_pool_S64 = ev->d_pool_S64; L.d_pool_chi2 = ev->d_pool_chi2; L.d_pool_nmatch = ev->d_pool_nmatch;

@@ -150,7 +150,7 @@ cudaError_t launch_best_track(const BestLaunch &L, cudaStream_t s)
     A.g = L.g; A.grids = L.d_grids; A.axes = L.d_axes; A.axis_stride = L.axis_stride;
     A.drift_tab = L.d_drift_tab; A.bits = L.d_bits; A.W = L.W; A.n_bit_words = L.n_bit_words;
     A.h = L.h; A.lambda = L.window * L.window; A.eloss_h = L.eloss * L.h; A.kq = CDC_KAPPA * (double)L.charge;
-    A.max_steps = L.max_steps;
+    A.max_steps = L.max_steps; A.lookup_every = L.lookup_every64;
     cudaError_t e;
     if ((e = cudaMemsetAsync(L.d_ev_maxS, 0, sizeof(unsigned long long) * (size_t)L.n_events, s)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(L.d_ev_best, 0xFF, sizeof(unsigned long long) * (size_t)L.n_events, s)) != cudaSuccess) return e;

@@ -214,7 +214,7 @@ struct BestLaunch {
     const uint32_t *d_bits;
     int32_t W, n_bit_words, max_hits_per_event;
     double h, window, eloss;
-    int32_t max_steps, charge;
+    int32_t max_steps, charge, lookup_every64;
     float margin;
     const uint64_t *d_best_key;
     const PoolEntry *d_pool;
@@ -233,5 +233,8 @@ struct BestLaunch {
     int32_t *d_labels;
 };
 cudaError_t launch_best_track(const BestLaunch &L, cudaStream_t s);
+
+// K64: how many intervals the 3 x 3 candidate set of the fp64 evaluation stays a superset (reading C8)
+int32_t cdc_lookup_every64(const cdc_geometry *g, double h_mm, double window_mm);
 
 cudaError_t run_fp32_peak_probe(int32_t iters, double *flops_per_s, double *ms, cudaStream_t s);

@@ -18,6 +18,7 @@ struct BestArgs {
     int32_t W, n_bit_words;
     double h, lambda, eloss_h, kq;
     int32_t max_steps;
+    int32_t lookup_every;      // K64: steps per 3 x 3 candidate lookup
 };
 
 __device__ __forceinline__ void field64(const Geom64 &g, double x, double y, double z, double *B)
@@ -99,7 +100,7 @@ __device__ __forceinline__ int lane_candidate(const Geom64 &g, const LayerDev *s
     const float u2 = x * x + y * y - zeta * zeta;
     if (!(u2 > 0.0f) || lane >= 9) return -1;
     const float fj = (sqrtf(u2) - g.r_first) * g.inv_pitch;
-    if (fj < -1.0f || fj > (float)g.n_layers) return -1;
+    if (fj < -1.5f || fj > (float)g.n_layers + 0.5f) return -1;      // beyond the reach of any wire for K64 steps
     const int j = (int)rintf(fj) - 1 + lane / 3;
     if (j < 0 || j >= g.n_layers) return -1;
     const LayerDev L = s_layer[j];
@@ -138,22 +139,43 @@ __device__ void eval_seed64(const BestArgs &A, const LayerDev *s_layer, int e, i
     const float *drift = A.drift_tab + (size_t)he * A.W;
     int n = 0, turn = 0, m = 0, n_match = 0, n_rec = 0;
     bool cn = true;
+    int kc = 0, w = -1;
+    float wr[5] = {0.f, 0.f, 0.f, 0.f, 1.f};
+    double g0 = 0.0, drift_w = 0.0;
     double a = A.kq / p, p_of_a = p;
     while (n < A.max_steps) {
         if (p != p_of_a) { a = A.kq / p; p_of_a = p; }                  // a = kappa q / p_n (C5/C6)
         double rn[3], Tn[3];
+        // every K64 steps: this lane's candidate wire around r_n and g at r_n.  A wire outside the 3 x 3 set is at
+        // least 1.5 layer pitches / 1.5 cells away, so the set stays a superset of the wires that can own a match for
+        // K64 intervals (reading C8); g is carried from vertex to vertex (same operands, same value as a fresh
+        // evaluation), the wire record is held in registers.
+        if (kc == 0) {
+            kc = A.lookup_every;
+            w = lane_candidate(A.g, s_layer, bits, r, lane);
+            if (w >= 0) {
+                const float *wp = A.g.wire5 + (size_t)w * 5;
+#pragma unroll
+                for (int i = 0; i < 5; ++i) wr[i] = __ldg(wp + i);
+                drift_w = (double)__ldg(drift + w);
+                double d0[3], tp;
+                wire_offset64(wr, r, d0, &tp);
+                g0 = d0[0] * T[0] + d0[1] * T[1] + d0[2] * T[2];
+            }
+        }
+        kc -= 1;
         rkn_step64(A.g, a, A.h, r, T, rn, Tn);
+        double g1 = 0.0;
+        if (w >= 0) {
+            double d1[3], tp;
+            wire_offset64(wr, rn, d1, &tp);
+            g1 = d1[0] * Tn[0] + d1[1] * Tn[1] + d1[2] * Tn[2];
+        }
         if (cn) {
-            const int w = lane_candidate(A.g, s_layer, bits, r, lane);
             bool matched = false;
             double r2 = 0.0, ad = 0.0;
             if (w >= 0) {
-                const float *wr = A.g.wire5 + (size_t)w * 5;
-                double d0[3], d1[3], tp;
-                wire_offset64(wr, r, d0, &tp);
-                const double g0 = d0[0] * T[0] + d0[1] * T[1] + d0[2] * T[2];
-                wire_offset64(wr, rn, d1, &tp);
-                const double g1 = d1[0] * Tn[0] + d1[1] * Tn[1] + d1[2] * Tn[2];
+                double tp;
                 if (g0 <= 0.0 && g1 > 0.0) {
                     const double tau = g0 / (g0 - g1);
                     double P[3], d[3];
@@ -162,7 +184,7 @@ __device__ void eval_seed64(const BestArgs &A, const LayerDev *s_layer, int e, i
                     wire_offset64(wr, P, d, &tp);
                     const double D = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
                     const double zw = tp * (double)wr[4];
-                    const double resid = D - (double)__ldg(drift + w);
+                    const double resid = D - drift_w;
                     r2 = resid * resid; ad = fabs(resid);
                     matched = fabs(zw) <= A.g.z_half && r2 < A.lambda;
                 }
@@ -187,6 +209,7 @@ __device__ void eval_seed64(const BestArgs &A, const LayerDev *s_layer, int e, i
             }
             m += 1;
         }
+        g0 = g1;
 #pragma unroll
         for (int i = 0; i < 3; ++i) { r[i] = rn[i]; T[i] = Tn[i]; }
         n += 1;

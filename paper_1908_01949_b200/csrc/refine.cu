@@ -196,7 +196,7 @@ BestArgs make_args(const RefineLaunch &L, const GridDev *grids, const double *ax
     A.g = L.g; A.grids = grids; A.axes = axes; A.axis_stride = stride;
     A.drift_tab = L.d_drift_tab; A.bits = L.d_bits; A.W = L.W; A.n_bit_words = L.n_bit_words;
     A.h = L.h; A.lambda = L.window * L.window; A.eloss_h = L.eloss * L.h; A.kq = CDC_KAPPA * (double)L.charge;
-    A.max_steps = L.max_steps;
+    A.max_steps = L.max_steps; A.lookup_every = L.lookup_every64;
     return A;
 }
 

@@ -21,7 +21,7 @@ struct RefineLaunch {
     const int32_t *d_offsets, *d_wire_id;
     int32_t W, n_bit_words, max_hits_per_event;
     double h, window, eloss;
-    int32_t max_steps, charge;
+    int32_t max_steps, charge, lookup_every64;
     uint32_t *d_cand_idx;            // [E][cap]
     int32_t *d_count;                // [E]: candidates (iteration 0) or parents (iterations >= 1)
     double *d_S64, *d_chi2_64;       // [E][cap]
