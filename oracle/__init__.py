@@ -154,10 +154,11 @@ def scan(bound: Bound, wire_id, drift, grid, begin: int = 0, end: Optional[int] 
     ns = np.zeros(n, dtype=np.int32) if details else None
     tu = np.zeros(n, dtype=np.int32) if details else None
     fr = np.zeros((n, 3)) if details else None
+    mg = np.zeros(n, dtype=np.int32) if details else None
     lib().orc_scan(C.byref(bound.g), C.byref(bound.f), C.byref(H), _p(lo), _p(st), _p(nn), _p(il),
                    C.c_int64(begin), C.c_int64(end), C.byref(bound.P), C.c_int32(mode),
-                   _p(nm), _p(c2), _p(ns), _p(tu), _p(fr))
-    return dict(n_match=nm, chi2=c2, n_steps=ns, turns=tu, final_r=fr)
+                   _p(nm), _p(c2), _p(ns), _p(tu), _p(fr), _p(mg))
+    return dict(n_match=nm, chi2=c2, n_steps=ns, turns=tu, final_r=fr, m_gas=mg)
 
 
 def _scan_worker(args):

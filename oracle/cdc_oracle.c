@@ -299,7 +299,8 @@ void orc_scan(const orc_geom *g, const orc_field *f, const orc_hits *hits,
               const double *lo, const double *step, const int32_t *nn,
               const int64_t *index_list /* or NULL */, int64_t begin, int64_t end,
               const orc_params *P, int32_t mode,
-              int32_t *n_match, double *chi2, int32_t *n_steps, int32_t *turns, double *final_r /* [..][3] */)
+              int32_t *n_match, double *chi2, int32_t *n_steps, int32_t *turns, double *final_r /* [..][3] */,
+              int32_t *m_gas /* or NULL: in-gas steps (reading C6) */)
 {
     int32_t *how = (int32_t *)malloc(sizeof(int32_t) * (size_t)g->n_wires_total);
     int64_t s;
@@ -316,6 +317,7 @@ void orc_scan(const orc_geom *g, const orc_field *f, const orc_hits *hits,
         n_match[o] = res.n_match; chi2[o] = res.chi2;
         if (n_steps) n_steps[o] = res.n_steps;
         if (turns) turns[o] = res.turns;
+        if (m_gas) m_gas[o] = res.m_gas;
         if (final_r) { final_r[3 * o] = res.r[0]; final_r[3 * o + 1] = res.r[1]; final_r[3 * o + 2] = res.r[2]; }
     }
     free(how);

@@ -32,6 +32,7 @@ struct ScanArgs {
     const uint32_t *bits;
     float h, h_half, h2_8, h2_2, h_6, h2_6;
     double kq;                 // kappa * charge
+    float kq_rel;              // kq / fl32(kq) - 1: the systematic part of a = fl32(kq) / p (energy-loss path)
     double h6_64;              // h / 6 in fp64 (for the systematic-rounding correction)
     float lambda, inv_lambda, eloss_h;
     float u2_lo, u2_hi;        // lookup band in u^2, widened by (K - 1) h
@@ -235,6 +236,7 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
     const uint32_t index = (uint32_t)((((i_th * G.n[1] + i_z) * G.n[2] + i_px) * G.n[3] + i_py) * G.n[4] + i_pz);
 
     float xh, xl, yh, yl, zh, zl, Txh, Txl, Tyh, Tyl, Tzh, Tzl, a, epsT, p0h, p0l;
+    float ub_h = 0.f, ub_l = 0.f, ue1 = 0.f, up1 = 0.f, up2_h = 0.f, up2_l = 0.f;   // uniform-field step map (FIELD == 0)
     {
         const double *ax = A.axes + (size_t)e * 6 * A.axis_stride;
         double x0 = ax[i_th], y0 = ax[A.axis_stride + i_th], z0 = ax[2 * A.axis_stride + i_z];
@@ -251,7 +253,17 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
         a = (float)a64;
         // the fp32 roundings of a and h/6 are the same every step; fold their ratio into the T update
         epsT = (float)((a64 * A.h6_64) / ((double)a * (double)A.h_6) - 1.0);
+        // with energy loss a is recomputed every step as fl32(kq) / p: the systematic roundings are those of kq and h/6
+        if (ELOSS) epsT = (float)((A.kq * A.h6_64) / ((double)(float)A.kq * (double)A.h_6) - 1.0);
         p0h = (float)p0; p0l = (float)(p0 - (double)p0h);
+        if (FIELD == 0) {                              // step-map constants in fp64, the two O(theta) ones as hi + lo
+            const double h64 = 6.0 * A.h6_64, th = a64 * (double)A.fd.bz * h64, th2 = th * th;
+            const double b = th - th * th2 / 6.0, p2 = h64 * (th / 2.0 - th * th2 / 24.0);
+            ub_h = (float)b; ub_l = (float)(b - (double)ub_h);
+            up2_h = (float)p2; up2_l = (float)(p2 - (double)up2_h);
+            ue1 = (float)(-th2 / 2.0 + th2 * th2 / 24.0);
+            up1 = (float)(-h64 * th2 / 6.0);
+        }
     }
     const bool low_p = !(p0h > 1.0f);                 // p <= 1 MeV/c ends a track after its first step (C7)
 
@@ -295,24 +307,27 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
 
         // ---- A4: one Nystroem-RK4 step of r'' = a (r' x B(r))
         if (FIELD == 0) {
-            // uniform field B = (0, 0, Bz): k = a Bz (T_y, -T_x, 0); k_z == 0, T_z constant, no stage positions needed
-            const float c = a * A.fd.bz;
-            const float k1x = c * Tyh, k1y = -c * Txh;
-            float Ux = fmaf(A.h_half, k1x, Txh), Uy = fmaf(A.h_half, k1y, Tyh);
-            const float k2x = c * Uy, k2y = -c * Ux;
-            Ux = fmaf(A.h_half, k2x, Txh); Uy = fmaf(A.h_half, k2y, Tyh);
-            const float k3x = c * Uy, k3y = -c * Ux;
-            Ux = fmaf(h, k3x, Txh); Uy = fmaf(h, k3y, Tyh);
-            const float k4x = c * Uy, k4y = -c * Ux;
-            const float dx = fmaf(A.h2_6, (k1x + k2x) + k3x, h * Txh);
-            const float dy = fmaf(A.h2_6, (k1y + k2y) + k3y, h * Tyh);
-            const float dTx = A.h_6 * fmaf(2.0f, k2x + k3x, k1x + k4x);
-            const float dTy = A.h_6 * fmaf(2.0f, k2y + k3y, k1y + k4y);
-            comp_add(xh, xl, fmaf(h, Txl, dx));        // h * T_lo: the part of T the fp32 stages never saw
+            // uniform field B = (0, 0, Bz): the four stages are linear in T, k = c J U with J (Tx, Ty) = (Ty, -Tx), so
+            // the Nystroem step collapses (exactly, theta = a Bz h) to
+            //   dT = [ (theta - theta^3/6) J + (-theta^2/2 + theta^4/24) I ] T
+            //   dr = h T + h [ (theta/2 - theta^3/24) J - (theta^2/6) I ] T          (k_z == 0, T_z constant)
+            // -- the same map as k1..k4 and the weighted sums, with the stage arithmetic done once per seed.
+            if (ELOSS) {                                  // theta follows p_n; constants in fp32 like a itself
+                const float th = a * A.fd.bz * h, th2 = th * th;
+                ub_h = fmaf(-th * th2, 0.166666672f, th); ub_l = ub_h * A.kq_rel;      // fl(kappa q) is off by the same
+                ue1 = th2 * fmaf(th2, 0.0416666679f, -0.5f);                           // relative amount every step
+                up1 = -h * th2 * 0.166666672f;
+                up2_h = h * th * fmaf(th2, -0.0416666679f, 0.5f); up2_l = up2_h * A.kq_rel;
+            }
+            const float dTx = fmaf(ue1, Txh, fmaf(ub_h, Tyh, ub_l * Tyh));
+            const float dTy = fmaf(ue1, Tyh, -fmaf(ub_h, Txh, ub_l * Txh));
+            const float dx = fmaf(up1, Txh, fmaf(up2_h, Tyh, fmaf(up2_l, Tyh, h * Txh)));
+            const float dy = fmaf(up1, Tyh, -fmaf(up2_h, Txh, fmaf(up2_l, Txh, -h * Tyh)));
+            comp_add(xh, xl, fmaf(h, Txl, dx));        // h * T_lo: the part of T the fp32 products never saw
             comp_add(yh, yl, fmaf(h, Tyl, dy));
             comp_add(zh, zl, fmaf(h, Tzl, h * Tzh));
-            comp_add(Txh, Txl, fmaf(dTx, epsT, dTx));
-            comp_add(Tyh, Tyl, fmaf(dTy, epsT, dTy));
+            comp_add(Txh, Txl, dTx);
+            comp_add(Tyh, Tyl, dTy);
         } else {
             float Bx, By, Bz;
             field_at<FIELD>(A.fd, xh, yh, zh, Bx, By, Bz);
@@ -442,6 +457,7 @@ cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0
     A.h = (float)h; A.h_half = (float)(h / 2.0); A.h2_8 = (float)(h * h / 8.0); A.h2_2 = (float)(h * h / 2.0);
     A.h_6 = (float)(h / 6.0); A.h2_6 = (float)(h * h / 6.0);
     A.kq = CDC_KAPPA * (double)L.charge; A.h6_64 = h / 6.0;
+    A.kq_rel = (float)(A.kq / (double)(float)A.kq - 1.0);
     A.lambda = L.lambda; A.inv_lambda = 1.0f / L.lambda; A.eloss_h = L.eloss_h;
     A.u2_lo = L.u2_lo; A.u2_hi = L.u2_hi; A.uz = L.uz; A.inv_uz = L.inv_uz; A.lookup_every = L.lookup_every;
     A.delta_max = L.delta_max; A.b_max = L.b_max; A.hold_path = L.hold_path;

@@ -54,7 +54,10 @@ def compare_scan(cfg, geom, field, ev, grid, gpu, orc, sel, offset=0):
     dbg = gpu["debug"][offset + sel]
     nm_g = gpu["n_match"][offset + sel]
     c2_g = gpu["chi2"][offset + sel]
-    same_steps = dbg["n_steps"] == orc["n_steps"]
+    # same number of steps and -- with energy loss -- of in-gas steps: the momentum, hence the track, is defined
+    # through that integer (reading C6), so a start vertex within 1e-3 mm of R0 (SURVEY 8(d) parity procedure (ii),
+    # listed exception class) changes the rest of the track
+    same_steps = (dbg["n_steps"] == orc["n_steps"]) & (dbg["m_gas"] == orc["m_gas"])
     pos = np.stack([dbg["x"], dbg["y"], dbg["z"]], axis=1)
     err = np.linalg.norm(pos - orc["final_r"], axis=1)
     assert err[same_steps].max() < POS_TOL_MM, f"position error {err[same_steps].max()} mm"
