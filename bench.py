@@ -271,6 +271,8 @@ def run_ours(args):
                 "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s",
                              "frac": achieved / PEAK_FP32_TFLOPS, "traffic": measured_traffic(args.workload), "kernel": "seed_scan_kernel",
                              "flops_per_rkn_step": flops / max(acc["n_steps"], 1),
+                             "note": "flops = the step as the method defines it (DESIGN.md section 7); the uniform-field "
+                                     "kernel executes its closed form, 56 instead of 78 flops per step",
                              "peak_source": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (nominal, B200_PROFILING.md)"}}
         f, _ = B.cdc_fp32_peak_probe(4096)
         line["roofline"]["ffma_probe_tflops"] = f / 1e12
