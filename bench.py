@@ -58,6 +58,9 @@ def parse():
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE.json configs[4]: throughput of the scan over grid size, batch size and step size "
                          "(one JSON line per point; not the driver's bench line)")
+    ap.add_argument("--paper-mapping", action="store_true",
+                    help="measure the re-created thread mapping of the paper (one block per seed, one thread per fired "
+                         "wire) against the product kernel on a sample of the workload's seeds (comparison point)")
     return ap.parse_args()
 
 
@@ -325,9 +328,45 @@ def run_sweep(args):
         ev.close()
 
 
+def run_paper_mapping(args):
+    """seeds/s of the paper's v1 mapping on this GPU, same event, same grid, a stratified
+    sample of the seeds; the product kernel is timed on the whole grid."""
+    import torch
+    from paper_1908_01949_b200 import api, binding as B
+    torch.cuda.set_device(0)
+    cfg_id, cfg, geom, field, events, grids = make_workload(args, 0)
+    sc = api.SeedScanner(geom, field)
+    off, w, d = synth.pack_hits(events)
+    ev = B.Events(sc.geometry, off, w, d)
+    P = B.scan_params(cfg.h_mm, cfg.max_steps, cfg.window_mm)
+    n = 8192
+    sel = synth.stratified_seed_sample(grids[0].n_seeds, n, key=4)
+    d_sel = torch.tensor(sel, dtype=torch.int64, device="cuda")
+    d_nm = torch.zeros(n, dtype=torch.int32, device="cuda"); d_c2 = torch.zeros(n, dtype=torch.float32, device="cuda")
+    ms = []
+    for it in range(3):
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); e0.record()
+        B.cdc_seed_scan_paper_mapping(sc.geometry, ev, 0, grids[0], P, d_sel, d_nm, d_c2)
+        e1.record(); e1.synchronize()
+        if it:
+            ms.append(e0.elapsed_time(e1))
+    d_key = torch.zeros(len(events), dtype=torch.int64, device="cuda")
+    for it in range(3):
+        B.cdc_seed_scan(sc.geometry, ev, B.grid_specs(grids), P, d_key)
+        st = B.cdc_scan_get_stats(ev)
+    t_v1 = float(np.mean(ms)) * 1e-3
+    ours = st["n_seeds"] / (st["kernel_ms"] * 1e-3)
+    print(json.dumps({"comparison": "paper_v1_mapping", "workload": args.workload, "hits": int(off[1]), "sample_seeds": n,
+                      "paper_mapping_ms": t_v1 * 1e3, "paper_mapping_seeds_per_s": n / t_v1,
+                      "product_kernel_seeds_per_s": ours, "ratio": ours / (n / t_v1)}))
+
+
 if __name__ == "__main__":
     a = parse()
-    if a.sweep:
+    if a.paper_mapping:
+        run_paper_mapping(a)
+    elif a.sweep:
         run_sweep(a)
     else:
         run_reference(a) if a.impl == "reference" else run_ours(a)

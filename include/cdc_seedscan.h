@@ -215,6 +215,15 @@ int32_t cdc_classification_quality(const cdc_events *ev, int32_t n_turns, const 
 int32_t cdc_common_hits(const cdc_events *ev, const int32_t *d_labels_a, const int32_t *d_labels_b,
                         int32_t turn_a, int32_t turn_b, int32_t *d_n_common, void *stream);
 
+/* MEASURED COMPARISON POINT, not the product path: the paper's own thread mapping (v1, PAPER.md:73,
+ * Fig. 6) -- one block per seed, one thread per fired wire, every thread repeating the RKN propagation -- re-created on
+ * sm_100a with the same arithmetic and scoring rule as cdc_seed_scan.  Evaluates the n_seeds seeds d_seed_index[] (linear
+ * indices into h_grid) of one event; outputs d_n_match / d_chi2 [n_seeds].  No energy loss.  Asynchronous after an
+ * internal table copy. */
+int32_t cdc_seed_scan_paper_mapping(const cdc_geometry *g, cdc_events *ev, int32_t event, const cdc_grid_spec *h_grid,
+                                    const cdc_scan_params *params, const int64_t *d_seed_index, int32_t n_seeds,
+                                    uint32_t *d_n_match, float *d_chi2, void *stream);
+
 /* Number of kernels this library has launched in this process so far (bench.py's gpu_launches). */
 uint64_t cdc_kernel_launch_count(void);
 

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(HERE, "libcdc_seedscan.so")
 EXPORTS = ["cdc_last_error", "cdc_geometry_create", "cdc_geometry_destroy", "cdc_geometry_wire_table",
            "cdc_event_upload", "cdc_events_destroy", "cdc_events_tables", "cdc_hough_dims",
            "cdc_hough_seed_ranges", "cdc_seed_scan", "cdc_scan_get_stats", "cdc_best_track",
-           "cdc_find_tracks_host", "cdc_refine_tracks", "cdc_classification_quality", "cdc_common_hits", "cdc_fp32_peak_probe", "cdc_kernel_launch_count"]
+           "cdc_find_tracks_host", "cdc_refine_tracks", "cdc_classification_quality", "cdc_common_hits", "cdc_seed_scan_paper_mapping", "cdc_fp32_peak_probe", "cdc_kernel_launch_count"]
 
 
 class CdcError(RuntimeError):
@@ -291,6 +291,14 @@ def cdc_common_hits(events: Events, d_labels_a, d_labels_b, turn_a: int = -1, tu
                                  _dp(out), _stream(stream)))
     torch.cuda.synchronize()
     return out.cpu().numpy()
+
+
+def cdc_seed_scan_paper_mapping(geometry: Geometry, events: Events, event: int, grid, params: ScanParams, d_seed_index,
+                                d_n_match, d_chi2, stream=None):
+    """The paper's block-per-seed / thread-per-fired-wire mapping (comparison point only)."""
+    _check(lib().cdc_seed_scan_paper_mapping(geometry.handle, events.handle, C.c_int32(event), grid_specs([grid]),
+                                             C.byref(params), _dp(d_seed_index), C.c_int32(int(d_seed_index.numel())),
+                                             _dp(d_n_match), _dp(d_chi2), _stream(stream)))
 
 
 def cdc_kernel_launch_count() -> int:
