@@ -62,6 +62,23 @@ def test_cfg1_full_size_sampled(torch_cuda):
     print(f"cfg1: {len(listed)} listed threshold exceptions of {sel.size} sampled seeds")
 
 
+def test_cfg1_full_size_every_seed(torch_cuda):
+    """All 1,048,576 seeds of configs[1] against the oracle (split over the host cores by seed range; every process is
+    the single-threaded oracle): positions, step counts, n_match, chi2, turns; the oracle's argmax over the WHOLE grid."""
+    import os
+    cfg, geom, field, events, grids = U.make_workload(1, first_event=1)
+    ev, grid = events[0], grids[0]
+    sc = api.SeedScanner(geom, field)
+    gpu, off = _scan_all(sc, events, grids, cfg)
+    orc = oracle.scan_parallel(geom, field, U.oracle_params(cfg), ev.wire_id, ev.drift_mm, grid, n_proc=os.cpu_count())
+    listed = U.compare_scan(cfg, geom, field, ev, grid, gpu, orc, np.arange(grid.n_seeds))
+    U.check_best(cfg, geom, field, ev, grid, gpu, orc_full=orc)
+    S = orc["n_match"] - orc["chi2"] / cfg.window_mm ** 2
+    top2 = np.sort(S)[-2:]
+    print(f"cfg1 full grid: {len(listed)} listed threshold exceptions of {grid.n_seeds}; S gap of the two best seeds "
+          f"{top2[1] - top2[0]:.4f}")
+
+
 # ------------------------------------------------------------------ config 2: Hough ranges, energy loss, 24^5
 def _hough_edge_votes(geom, ev, zref, hp, bins):
     """Number of (hit, bin) pairs whose vote is within EDGE_TOL of the tolerance edge, for the listed bins."""
@@ -147,6 +164,13 @@ def test_cfg3_table_field_batch(torch_cuda):
     listed = 0
     for e, (ev, grid) in enumerate(zip(events, grids)):
         o = e * grid.n_seeds
+        if e == 0:          # one event of the batch in full: every seed, and the oracle's argmax over the whole grid
+            import os
+            sel = np.arange(grid.n_seeds)
+            orc = oracle.scan_parallel(geom, field, U.oracle_params(cfg), ev.wire_id, ev.drift_mm, grid, n_proc=os.cpu_count())
+            listed += len(U.compare_scan(cfg, geom, field, ev, grid, gpu, orc, sel, offset=o))
+            U.check_best(cfg, geom, field, ev, grid, gpu, e=e, hit_slice=slice(off[e], off[e + 1]), orc_full=orc)
+            continue
         sel = synth.stratified_seed_sample(grid.n_seeds, 250, key=100 + e)
         orc = oracle.scan_parallel(geom, field, U.oracle_params(cfg), ev.wire_id, ev.drift_mm, grid, index_list=sel)
         listed += len(U.compare_scan(cfg, geom, field, ev, grid, gpu, orc, sel, offset=o))
