@@ -105,7 +105,8 @@ typedef struct {
 typedef struct {
     uint64_t n_seeds;          /* seeds propagated */
     uint64_t n_steps;          /* RKN steps taken, summed over seeds */
-    uint64_t n_gas_steps;      /* of which started in the gas volume (rho >= R0) */
+    uint64_t n_gas_steps;      /* of which started in the gas volume (rho >= R0); counted only with energy loss or the
+                                  debug output (otherwise 0: the production kernel does not track the flag) */
     uint64_t n_approach_tests; /* live candidate wires examined (g evaluated) */
     uint64_t n_pool;           /* candidate-pool entries appended (reading C11) */
     uint64_t pool_cap;

@@ -130,7 +130,10 @@ __device__ __forceinline__ void slot_step(const ScanArgs &A, const float *drift_
     g = gn;
 }
 
-template <int FIELD, bool ELOSS>
+// TRACK: keep the in-gas flag, the in-gas step count and the turn counter.  They are needed with energy loss (p_n is
+// defined through m_n), for the debug record, and when a held wire could be scored from a vertex inside R0; otherwise
+// every vertex a wire can be scored from lies in the gas (host check in launch_seed_scan) and they are dead weight.
+template <int FIELD, bool ELOSS, bool TRACK>
 __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
 {
     __shared__ LayerDev s_layer[CDC_MAX_LAYERS];
@@ -189,7 +192,8 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
             up1 = (float)(-h64 * th2 / 6.0);
         }
     }
-    const bool low_p = !(p0h > 1.0f);                 // p <= 1 MeV/c ends a track after its first step (C7)
+    // p <= 1 MeV/c ends a track after its first step (C7)
+    const int max_steps = (p0h > 1.0f) ? A.max_steps : min(A.max_steps, 1);
 
     uint32_t nm = 0, tests = 0, cnt = 0, lookups = 0;
     float chi2 = 0.0f;
@@ -200,7 +204,7 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
     S.n = 0; S.w0 = S.w1 = S.w2 = S.w3 = 0; S.g0 = S.g1 = S.g2 = S.g3 = 0.0f;
 
 #pragma unroll 2
-    while (valid && n < A.max_steps) {
+    while (valid && n < max_steps) {
         // ---- A5: every K steps, the wires near r_n that carry a hit -> slots, with g at this vertex
         if (kcount == 0) {
             kcount = A.lookup_every;
@@ -298,14 +302,16 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
             if (S.n > 2) slot_step(A, drift_e, S.w2, S.g2, cn, v0, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
             if (S.n > 3) slot_step(A, drift_e, S.w3, S.g3, cn, v0, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
         }
-        if (cn) m += 1;
+        if (TRACK && cn) m += 1;
 
         // ---- advance, energy loss (reading C6), turn counter and termination (reading C7)
         n += 1;
         float rho2 = fmaf(xh, xh, yh * yh);
-        bool cnext = rho2 >= A.gd.R0sq;
-        if (!cn && cnext) turn += 1;
-        cn = cnext;
+        if (TRACK) {
+            bool cnext = rho2 >= A.gd.R0sq;
+            if (!cn && cnext) turn += 1;
+            cn = cnext;
+        }
         if (ELOSS) {
             float p = fmaf(-A.eloss_h, (float)m, p0h) + p0l;
             a = (float)A.kq / p;      // IEEE division
@@ -313,7 +319,6 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
         }
         if (!(fabsf(zh) <= A.gd.z_half)) break;
         if (!(rho2 <= A.gd.r_out_sq)) break;
-        if (low_p) break;
     }
 
     // ---- A7: per-seed output, per-event argmax, candidate pool
@@ -393,12 +398,18 @@ cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0
     dim3 grid((unsigned)((L.max_seeds_per_event + kBlock - 1) / kBlock), (unsigned)L.n_events);
     const bool eloss = L.eloss_h != 0.0f;
     if (k0) cudaEventRecord(k0, s);
+    // a held wire is scored from vertices at most (K - 1) h inside the lookup band's lower edge: if that is still outside
+    // R0 the in-gas flag is true whenever it is read (c_0 := true covers the start vertex)
+    const double u_lo = sqrt((double)L.u2_lo);
+    const bool track = eloss || L.d_debug != nullptr || !(u_lo - (L.lookup_every - 1) * h - 0.5 >= sqrt((double)L.gd.R0sq));
     if (L.fd.kind == 0) {
-        if (eloss) seed_scan_kernel<0, true><<<grid, kBlock, 0, s>>>(A);
-        else seed_scan_kernel<0, false><<<grid, kBlock, 0, s>>>(A);
+        if (eloss) seed_scan_kernel<0, true, true><<<grid, kBlock, 0, s>>>(A);
+        else if (track) seed_scan_kernel<0, false, true><<<grid, kBlock, 0, s>>>(A);
+        else seed_scan_kernel<0, false, false><<<grid, kBlock, 0, s>>>(A);
     } else {
-        if (eloss) seed_scan_kernel<1, true><<<grid, kBlock, 0, s>>>(A);
-        else seed_scan_kernel<1, false><<<grid, kBlock, 0, s>>>(A);
+        if (eloss) seed_scan_kernel<1, true, true><<<grid, kBlock, 0, s>>>(A);
+        else if (track) seed_scan_kernel<1, false, true><<<grid, kBlock, 0, s>>>(A);
+        else seed_scan_kernel<1, false, false><<<grid, kBlock, 0, s>>>(A);
     }
     if (k1) cudaEventRecord(k1, s);
     cdc_count_launch();

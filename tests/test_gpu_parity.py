@@ -73,6 +73,15 @@ def test_cfg1_full_size_every_seed(torch_cuda):
     orc = oracle.scan_parallel(geom, field, U.oracle_params(cfg), ev.wire_id, ev.drift_mm, grid, n_proc=os.cpu_count())
     listed = U.compare_scan(cfg, geom, field, ev, grid, gpu, orc, np.arange(grid.n_seeds))
     U.check_best(cfg, geom, field, ev, grid, gpu, orc_full=orc)
+    # the launch configuration bench.py times (no debug record: the kernel variant without the in-gas bookkeeping, no
+    # per-seed outputs either in the second call) gives bit-identical scores and the same best seed
+    off_, w_, d_ = synth.pack_hits(events)
+    E2 = sc.upload(off_, w_, d_)
+    fast = sc.scan(E2, grids, U.gpu_params(cfg), per_seed=True, debug=False)
+    assert np.array_equal(fast["n_match"], gpu["n_match"]) and np.array_equal(fast["chi2"], gpu["chi2"])
+    bare = sc.scan(E2, grids, U.gpu_params(cfg), per_seed=False, debug=False)
+    for k in ("best_seed", "best_n_match", "best_chi2", "labels", "best_key"):
+        assert np.array_equal(bare[k], gpu[k]) and np.array_equal(fast[k], gpu[k]), k
     S = orc["n_match"] - orc["chi2"] / cfg.window_mm ** 2
     top2 = np.sort(S)[-2:]
     print(f"cfg1 full grid: {len(listed)} listed threshold exceptions of {grid.n_seeds}; S gap of the two best seeds "
@@ -175,6 +184,11 @@ def test_cfg3_table_field_batch(torch_cuda):
         orc = oracle.scan_parallel(geom, field, U.oracle_params(cfg), ev.wire_id, ev.drift_mm, grid, index_list=sel)
         listed += len(U.compare_scan(cfg, geom, field, ev, grid, gpu, orc, sel, offset=o))
         U.check_best(cfg, geom, field, ev, grid, gpu, e=e, hit_slice=slice(off[e], off[e + 1]))
+    # the production launch configuration (no debug record -> kernel variant without the in-gas bookkeeping)
+    fast, _ = (sc.scan(sc.upload(*synth.pack_hits(events)), grids, U.gpu_params(cfg), per_seed=True, debug=False), None)
+    assert np.array_equal(fast["n_match"], gpu["n_match"]) and np.array_equal(fast["chi2"], gpu["chi2"])
+    for k in ("best_seed", "best_n_match", "best_chi2", "labels"):
+        assert np.array_equal(fast[k], gpu[k]), k
     print(f"cfg3: {listed} listed threshold exceptions; turns per event {[e.n_turns for e in events]}")
 
 
