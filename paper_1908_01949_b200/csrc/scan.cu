@@ -104,7 +104,7 @@ struct Vtx {               // position part of a step vertex (hi + the lo of x, 
 
 // One live wire over interval n: g at the far vertex; on g_n <= 0 < g_{n+1} the interval owns an approach (C9).
 __device__ __forceinline__ void slot_step(const ScanArgs &A, const float *drift_e, int w, float &g, bool score,
-                                          const Vtx &v0, const Vtx &v1, float Tx1, float Ty1, float Tz1,
+                                          float sdx, float sdy, float sdz, const Vtx &v1, float Tx1, float Ty1, float Tz1,
                                           uint32_t &nm, float &chi2, uint32_t &cnt)
 {
     const float4 wr = __ldg(A.gd.wire4 + w);
@@ -112,16 +112,17 @@ __device__ __forceinline__ void slot_step(const ScanArgs &A, const float *drift_
     const float gn = wire_g(wr, A.uz, A.inv_uz, v1.x, v1.xl, v1.y, v1.yl, v1.z, Tx1, Ty1, Tz1, ex1, ey1, eu1);
     if (score && g <= 0.0f && gn > 0.0f) {
         cnt += 1u << 16;
-        const float zt0 = __fmul_rn(v0.z, A.inv_uz);
-        const float ex0 = __fadd_rn(__fmaf_rn(-zt0, wr.z, __fsub_rn(v0.x, wr.x)), v0.xl);
-        const float ey0 = __fadd_rn(__fmaf_rn(-zt0, wr.w, __fsub_rn(v0.y, wr.y)), v0.yl);
-        const float tau = __fdividef(g, g - gn);
-        const float ex = fmaf(tau, ex1 - ex0, ex0);            // e is linear in the position: exact chord point
-        const float ey = fmaf(tau, ey1 - ey0, ey0);
+        // chord point P = r_{n+1} - (1 - tau)(r_{n+1} - r_n): e is linear in the position, and r_{n+1} - r_n is the
+        // increment (sdx, sdy, sdz) this step has just added, so e(P) follows from e_{n+1} without the old vertex
+        const float zd = sdz * A.inv_uz;
+        const float dex = fmaf(-zd, wr.z, sdx), dey = fmaf(-zd, wr.w, sdy);
+        const float sm = __fdividef(g, g - gn) - 1.0f;         // tau - 1, in [-1, 0)
+        const float ex = fmaf(sm, dex, ex1);
+        const float ey = fmaf(sm, dey, ey1);
         const float eu = fmaf(ex, wr.z, ey * wr.w);
         const float D2 = fmaf(ex, ex, fmaf(ey, ey, -eu * eu));
         const float D = sqrtf(fmaxf(D2, 0.0f));
-        const float zP = fmaf(tau, v1.z - v0.z, v0.z);
+        const float zP = fmaf(sm, sdz, v1.z);
         const float zw = fmaf(eu, A.uz, zP);
         const float resid = D - __ldg(drift_e + w);
         const float r2 = resid * resid;
@@ -230,8 +231,7 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
             }
         }
         kcount -= 1;
-        Vtx v0;
-        v0.x = xh; v0.xl = xl; v0.y = yh; v0.yl = yl; v0.z = zh;
+        float sdx, sdy, sdz;                           // the increment this step adds to the position
 
         // ---- A4: one Nystroem-RK4 step of r'' = a (r' x B(r))
         if (FIELD == 0) {
@@ -251,9 +251,10 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
             const float dTy = fmaf(ue1, Tyh, -fmaf(ub_h, Txh, ub_l * Txh));
             const float dx = fmaf(up1, Txh, fmaf(up2_h, Tyh, fmaf(up2_l, Tyh, h * Txh)));
             const float dy = fmaf(up1, Tyh, -fmaf(up2_h, Txh, fmaf(up2_l, Txh, -h * Tyh)));
-            comp_add(xh, xl, fmaf(h, Txl, dx));        // h * T_lo: the part of T the fp32 products never saw
-            comp_add(yh, yl, fmaf(h, Tyl, dy));
-            comp_add(zh, zl, fmaf(h, Tzl, h * Tzh));
+            sdx = fmaf(h, Txl, dx); sdy = fmaf(h, Tyl, dy); sdz = fmaf(h, Tzl, h * Tzh);   // h * T_lo: the part of T
+            comp_add(xh, xl, sdx);                                                         // the fp32 products never saw
+            comp_add(yh, yl, sdy);
+            comp_add(zh, zl, sdz);
             comp_add(Txh, Txl, dTx);
             comp_add(Tyh, Tyl, dTy);
         } else {
@@ -284,9 +285,10 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
             const float dTx = A.h_6 * fmaf(2.0f, k2x + k3x, k1x + k4x);
             const float dTy = A.h_6 * fmaf(2.0f, k2y + k3y, k1y + k4y);
             const float dTz = A.h_6 * fmaf(2.0f, k2z + k3z, k1z + k4z);
-            comp_add(xh, xl, fmaf(h, Txl, dx));
-            comp_add(yh, yl, fmaf(h, Tyl, dy));
-            comp_add(zh, zl, fmaf(h, Tzl, dz));
+            sdx = fmaf(h, Txl, dx); sdy = fmaf(h, Tyl, dy); sdz = fmaf(h, Tzl, dz);
+            comp_add(xh, xl, sdx);
+            comp_add(yh, yl, sdy);
+            comp_add(zh, zl, sdz);
             comp_add(Txh, Txl, fmaf(dTx, epsT, dTx));
             comp_add(Tyh, Tyl, fmaf(dTy, epsT, dTy));
             comp_add(Tzh, Tzl, fmaf(dTz, epsT, dTz));
@@ -297,10 +299,10 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
             Vtx v1;
             v1.x = xh; v1.xl = xl; v1.y = yh; v1.yl = yl; v1.z = zh;
             tests += (uint32_t)S.n;
-            slot_step(A, drift_e, S.w0, S.g0, cn, v0, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
-            if (S.n > 1) slot_step(A, drift_e, S.w1, S.g1, cn, v0, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
-            if (S.n > 2) slot_step(A, drift_e, S.w2, S.g2, cn, v0, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
-            if (S.n > 3) slot_step(A, drift_e, S.w3, S.g3, cn, v0, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
+            slot_step(A, drift_e, S.w0, S.g0, cn, sdx, sdy, sdz, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
+            if (S.n > 1) slot_step(A, drift_e, S.w1, S.g1, cn, sdx, sdy, sdz, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
+            if (S.n > 2) slot_step(A, drift_e, S.w2, S.g2, cn, sdx, sdy, sdz, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
+            if (S.n > 3) slot_step(A, drift_e, S.w3, S.g3, cn, sdx, sdy, sdz, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
         }
         if (TRACK && cn) m += 1;
 
