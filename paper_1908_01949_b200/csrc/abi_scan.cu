@@ -181,15 +181,24 @@ extern "C" int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cd
     L.margin = (float)(p->rescore_margin > 0.0 ? p->rescore_margin : kDefaultMargin);
     L.d_n_match = d_n_match; L.d_chi2 = d_chi2; L.d_debug = d_debug; L.d_best_key = d_best_key;
     L.d_pool = ev->d_pool; L.pool_cap = ev->pool_cap; L.d_counters = ev->d_counters;
-    // lookup cadence K: a wire that can own a match in interval n + i is within reach + i h of vertex n
+    // lookup cadence K: the 2 x 2 candidate set is taken around c = r_n + (K h / 2) T_n, the middle of the next K steps.
+    // A wire that can own a match in interval n + i lies within `reach` of vertex n + i, which lies within K h / 2 (+ the
+    // sagitta of that arc) of c; every wire outside the set is at least `excl` away from c (reading C8).
     {
         const double dmax = 8.0 + p->window_mm + 0.05;           // largest matching D: drift <= 8 mm (upload check)
         const double reach = sqrt(dmax * dmax + p->h_mm * p->h_mm) + 0.1;
         if (reach > g->excl) CDC_FAIL(CDC_ERR_RANGE, "cdc_seed_scan: window + step too large for the 2 x 2 wire lookup");
-        int K = 1 + (int)floor((g->excl - reach) / p->h_mm);
-        K = std::max(1, std::min(K, 8));
-        L.lookup_every = K;
-        const double grow = reach + 0.2 + (K - 1) * p->h_mm;
+        const double sag = 0.15;                                 // (K h / 2)^2 / (2 R) for R >= 150 mm, K h / 2 <= 6.7 mm
+        int K = (int)floor(2.0 * (g->excl - reach - sag) / p->h_mm);
+        K = std::max(1, std::min(K, 16));
+        double ahead = 0.5 * K * p->h_mm;
+        if (ahead + reach + sag > g->excl) { K = 1; ahead = 0.0; }
+        L.lookup_every = K; L.lookahead = (float)ahead;
+        // the straight-line prediction of the centre needs a track radius well above K h (the kernel checks
+        // |a| B_max < 1 / 20 mm per seed); tighter curls look up around r_n itself, every K0 steps
+        const int K0 = std::max(1, std::min(1 + (int)floor((g->excl - reach) / p->h_mm), 16));
+        L.lookup_every_tight = K0;
+        const double grow = reach + 0.2 + std::max(ahead + sag, (K0 - 1) * p->h_mm);
         const double ulo = std::max(g->r[0] - grow, 0.0), uhi = g->r[g->n_layers - 1] + grow;
         L.u2_lo = (float)(ulo * ulo); L.u2_hi = (float)(uhi * uhi);
         L.uz = g->uz; L.inv_uz = (float)(1.0 / (double)g->uz);
@@ -197,9 +206,9 @@ extern "C" int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cd
         // the track has moved at most K h since: |delta| <= diag + K h; it stays held while the track crosses
         // that neighbourhood, at most ~(diag + K h) / min|T_perp| of path -- bounded here by 4 diag
         const double diag = hypot(2.0 * g->pitch, 2.0 * g->cell_max);
-        L.delta_max = (float)(diag + K * p->h_mm + 1.0);
+        L.delta_max = (float)(diag + std::max(K, K0) * p->h_mm + 1.0);
         L.b_max = (float)(1.001 * g->b_max);
-        L.hold_path = (float)(4.0 * diag + 2.0 * K * p->h_mm);
+        L.hold_path = (float)(4.0 * diag + 2.0 * std::max(K, K0) * p->h_mm);
     }
     L.max_seeds_per_event = 0;
     for (const GridDev &G : ev->h_grids) L.max_seeds_per_event = std::max<int64_t>(L.max_seeds_per_event, G.n_seeds);

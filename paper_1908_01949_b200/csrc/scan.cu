@@ -39,7 +39,8 @@ struct ScanArgs {
     float u2_lo, u2_hi;        // lookup band in u^2, widened by (K - 1) h
     float uz, inv_uz;          // cos(eps) of the canonical wire table (one |stereo| for all layers)
     float delta_max, b_max, hold_path;   // bounds behind g_dead (see consider())
-    int32_t max_steps, lookup_every;
+    int32_t max_steps, lookup_every, lookup_every_tight;
+    float lookahead;
     float margin;
     uint32_t *n_match;
     float *chi2;
@@ -64,7 +65,8 @@ __device__ __forceinline__ void slot_push(Slots &S, int w, float g)
 }
 
 struct LookupCtx {         // the vertex a lookup is made from
-    float x, xl, y, yl, z, Tx, Ty, Tz, phi, g_dead;
+    float x, xl, y, yl, z, Tx, Ty, Tz;     // the vertex itself: g of a new slot is evaluated here
+    float cz, phi, g_dead;                 // height and azimuth of the lookup centre
 };
 
 // a candidate with a hit becomes a live slot unless the track has already passed it for good: once g exceeds
@@ -85,7 +87,7 @@ __device__ __forceinline__ void lookup_layer(const ScanArgs &A, const LayerDev *
 {
     if ((unsigned)j >= (unsigned)A.gd.n_layers) return;
     const LayerDev L = s_layer[j];
-    const float phi = V.phi, z = V.z;
+    const float phi = V.phi, z = V.cz;
     const float tau = z * L.shift_k;
     const float sh = fmaf(-0.333333343f * tau * tau, tau, tau);      // atan(tau), |tau| < 0.1
     const float kf = (phi - L.phi0 - sh) * L.kscale;
@@ -208,10 +210,15 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
     while (valid && n < max_steps) {
         // ---- A5: every K steps, the wires near r_n that carry a hit -> slots, with g at this vertex
         if (kcount == 0) {
-            kcount = A.lookup_every;
+            // centre of the next K steps (straight-line prediction; the arc's sagitta is in the host's margin); a seed
+            // curling tighter than 20 mm looks up around its own position instead, at the shorter cadence
+            const bool tight = !(fabsf(a) * A.b_max < 0.05f);
+            kcount = tight ? A.lookup_every_tight : A.lookup_every;
+            const float ahead = tight ? 0.0f : A.lookahead;
             S.n = 0;
-            const float zeta = zh * A.gd.tan_abs;
-            const float u2 = fmaf(xh, xh, fmaf(yh, yh, -zeta * zeta));
+            const float cx = fmaf(ahead, Txh, xh), cy = fmaf(ahead, Tyh, yh), cz = fmaf(ahead, Tzh, zh);
+            const float zeta = cz * A.gd.tan_abs;
+            const float u2 = fmaf(cx, cx, fmaf(cy, cy, -zeta * zeta));
             if (u2 > A.u2_lo && u2 < A.u2_hi) {
                 lookups += 1u;
                 const float u = u2 * rsqrtf(u2);
@@ -221,7 +228,8 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
                 const int j2 = jc + ((fj - jn) >= 0.0f ? 1 : -1);
                 LookupCtx V;
                 V.x = xh; V.xl = xl; V.y = yh; V.yl = yl; V.z = zh; V.Tx = Txh; V.Ty = Tyh; V.Tz = Tzh;
-                V.phi = coarse_atan2(yh, xh);
+                V.cz = cz;
+                V.phi = coarse_atan2(cy, cx);
                 {
                     const float cbend = (ELOSS ? 1.05f : 1.0f) * A.delta_max * fabsf(a) * A.b_max;
                     V.g_dead = fmaf(A.hold_path * 0.25f, cbend * cbend, 0.02f);
@@ -390,7 +398,7 @@ cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0
     A.kq = CDC_KAPPA * (double)L.charge; A.h6_64 = h / 6.0;
     A.kq_rel = (float)(A.kq / (double)(float)A.kq - 1.0);
     A.lambda = L.lambda; A.inv_lambda = 1.0f / L.lambda; A.eloss_h = L.eloss_h;
-    A.u2_lo = L.u2_lo; A.u2_hi = L.u2_hi; A.uz = L.uz; A.inv_uz = L.inv_uz; A.lookup_every = L.lookup_every;
+    A.u2_lo = L.u2_lo; A.u2_hi = L.u2_hi; A.uz = L.uz; A.inv_uz = L.inv_uz; A.lookup_every = L.lookup_every; A.lookahead = L.lookahead; A.lookup_every_tight = L.lookup_every_tight;
     A.delta_max = L.delta_max; A.b_max = L.b_max; A.hold_path = L.hold_path;
     A.max_steps = L.max_steps; A.margin = L.margin;
     A.n_match = L.d_n_match; A.chi2 = L.d_chi2; A.debug = L.d_debug;
@@ -400,10 +408,11 @@ cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0
     dim3 grid((unsigned)((L.max_seeds_per_event + kBlock - 1) / kBlock), (unsigned)L.n_events);
     const bool eloss = L.eloss_h != 0.0f;
     if (k0) cudaEventRecord(k0, s);
-    // a held wire is scored from vertices at most (K - 1) h inside the lookup band's lower edge: if that is still outside
+    // a held wire is scored from vertices at most `back` inside the lookup band's lower edge: if that is still outside
     // R0 the in-gas flag is true whenever it is read (c_0 := true covers the start vertex)
     const double u_lo = sqrt((double)L.u2_lo);
-    const bool track = eloss || L.d_debug != nullptr || !(u_lo - (L.lookup_every - 1) * h - 0.5 >= sqrt((double)L.gd.R0sq));
+    const double back = std::max((double)L.lookahead + 0.2, (L.lookup_every_tight - 1) * h);
+    const bool track = eloss || L.d_debug != nullptr || !(u_lo - back - 0.5 >= sqrt((double)L.gd.R0sq));
     if (L.fd.kind == 0) {
         if (eloss) seed_scan_kernel<0, true, true><<<grid, kBlock, 0, s>>>(A);
         else if (track) seed_scan_kernel<0, false, true><<<grid, kBlock, 0, s>>>(A);
