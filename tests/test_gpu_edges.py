@@ -201,3 +201,31 @@ def test_paper_thread_mapping_gives_the_same_scores(cfg_id):
     for i in np.nonzero(nm != orc["n_match"])[0]:
         assert U.explain_mismatch(bound, events[1], grids[1].node(grids[1].unravel(int(sel[i]))), cfg, geom)
     assert (nm != orc["n_match"]).sum() <= 2
+
+
+def test_tightly_curling_seeds_use_the_short_lookup_cadence(setup):
+    """Seeds with a track radius below 20 mm (|a| B >= 0.05 / mm) cannot use the look-ahead lookup centre; they fall
+    back to a lookup around their own position.  Every wire of the two innermost layers is fired, so any wire the
+    candidate set missed would show up as a missing match."""
+    cfg, geom, field, events, grids, sc = setup
+    w = np.arange(0, int(geom.offset[2]), dtype=np.int32)
+    d = np.full(w.size, 4.0, dtype=np.float32)
+    off = np.array([0, w.size], dtype=np.int32)
+    E = sc.upload(off, w, d)
+    # p between 3.5 and 6.5 MeV/c (radius 10-20 mm), pointing outward at R0 + a bit, mostly transverse
+    g = synth.Grid(lo=np.array([0.2, -50.0, 3.0, 1.0, 0.2]), step=np.array([0.9, 40.0, 0.6, 0.5, 0.15]),
+                   n=np.array([3, 3, 4, 4, 3], dtype=np.int32))
+    geom2 = synth.make_geometry(R0=522.0)                     # start close to the first layer so the curl reaches it
+    sc2 = api.SeedScanner(geom2, field)
+    E2 = sc2.upload(off, w, d)
+    P = B.scan_params(cfg.h_mm, 600, cfg.window_mm)
+    gpu = sc2.scan(E2, [g], P, per_seed=True, debug=True, best=False)
+    params = dict(h=cfg.h_mm, max_steps=600, window=cfg.window_mm)
+    orc = oracle.scan_parallel(geom2, field, params, w, d, g)
+    assert orc["n_match"].max() >= 3                          # the curls do reach fired wires
+    bound = oracle.Bound(geom2, field, params)
+    bad = np.nonzero((gpu["n_match"] != orc["n_match"]) | (gpu["debug"]["n_steps"] != orc["n_steps"]))[0]
+    for i in bad:
+        ev = synth.Event(wire_id=w, drift_mm=d, truth_turn=np.zeros_like(w), seed=np.zeros(5), n_turns=1, n_signal=0)
+        assert U.explain_mismatch(bound, ev, g.node(g.unravel(int(i))), cfg, geom2)
+    assert bad.size <= 3
