@@ -285,6 +285,18 @@ def run_ours(args):
             line["cpu_baseline"] = {"value": n / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                                     "sample": f"{n} stratified seeds of event 0 ({st} RKN steps, {dt:.1f} s)",
                                     "rkn_steps_per_s": st / dt}
+            # the same oracle as N independent single-threaded processes over disjoint seed ranges
+            import oracle
+            ncore = os.cpu_count() or 1
+            sel = synth.stratified_seed_sample(grids[0].n_seeds, 4 * n, 78)
+            t0 = time.perf_counter()
+            o = oracle.scan_parallel(geom, field, dict(h=cfg.h_mm, max_steps=cfg.max_steps, window=cfg.window_mm,
+                                                       eloss=cfg.eloss_MeV_per_mm), events[0].wire_id, events[0].drift_mm,
+                                     grids[0], index_list=sel, n_proc=ncore)
+            dtn = time.perf_counter() - t0
+            line["cpu_baseline"]["all_cores"] = {"value": sel.size / dtn, "unit": UNIT, "cores": ncore,
+                                                 "rkn_steps_per_s": int(o["n_steps"].sum()) / dtn,
+                                                 "sample": f"{sel.size} stratified seeds over {ncore} processes ({dtn:.1f} s)"}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -6,15 +6,15 @@
 //
 //   PAPER.md:51      seed (theta0, z0, px0, py0, pz0) at R0                     -> kernel prologue
 //   PAPER.md:55      RKN propagation (textbook Nystroem scheme, reading C5)     -> step body
-//   PAPER.md:55,:69  DCA to fired wires, sign-change ownership (reading C9)     -> wire_g(), score_approach()
+//   PAPER.md:55,:69  DCA to fired wires, sign-change ownership (reading C9)     -> wire_g(), slot_step()
 //   PAPER.md:65-69   Eq. (1): S = sum (1 - d^2/lambda) over matched terms       -> kernel epilogue
 //   PAPER.md:69      lowest E (= highest S) wins                                -> packed-key atomicMax
 //
-// Scoring structure (r1b): the layer/cell lookup runs once every K steps (K from the step size: the 2 x 2
-// candidate set of a vertex stays a superset of the wires that can own an approach for K intervals, reading
-// C8); the candidates that carry a hit are compacted into up to four per-thread slots (wire id + g at the
-// current vertex), so each step evaluates g once per live wire and runs the approach code only on a sign
-// change.
+// Scoring structure: the layer/cell lookup runs once every K steps around the middle of the next K steps (K from
+// the step size: the 2 x 2 candidate set of that point stays a superset of the wires that can own an approach for
+// K intervals, reading C8); the candidates that carry a hit are compacted into up to four per-thread slots (wire
+// id + g at the current vertex), so each step evaluates g once per live wire and runs the approach code only on a
+// sign change.  Lanes of a warp are seeds that differ in z0 first: they cross the same wires together.
 #include "cdc_internal.cuh"
 #include "scan_common.cuh"
 
