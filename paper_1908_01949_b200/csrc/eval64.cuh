@@ -49,12 +49,36 @@ __device__ __forceinline__ void lorentz64(double a, const double *T, const doubl
     k[2] = a * (T[0] * B[1] - T[1] * B[0]);
 }
 
-// reading C5: the four stages and the update, each expression evaluated left to right
-__device__ void rkn_step64(const Geom64 &g, double a, double h, const double *r, const double *T, double *rn,
-                           double *Tn)
+// reading C5: the four stages and the update, each expression evaluated left to right.
+// UNI (uniform field B = (0, 0, bz), position-independent): the same formulas with the terms that are exactly zero
+// left out.  x * 0 = +-0 and y -+ 0 = y in IEEE arithmetic, so every value equals the general form's (a zero may carry
+// the other sign, which no later operation can see: there is no division by, or sign test of, these quantities):
+//   k_x = a (T_y bz),  k_y = a (-(T_x bz)),  k_z = 0  ->  U_z = T_z,  T_z' = T_z,  z' = z + h T_z,
+// and the intermediate points q are never formed (nothing reads them).  37 % of the general form's instructions and a
+// dependent chain of 17 instead of 27 operations: the re-score is latency-bound.
+template <bool UNI>
+__device__ __forceinline__ void rkn_step64(const Geom64 &g, double a, double h, const double *r, const double *T,
+                                           double *rn, double *Tn)
 {
-    double B[3], k1[3], k2[3], k3[3], k4[3], q[3], U[3];
     const double hh = h / 2.0, h28 = h * h / 8.0, h22 = h * h / 2.0, h26 = h * h / 6.0, h6 = h / 6.0;
+    if (UNI) {
+        const double bz = g.bz;
+        const double k1x = a * (T[1] * bz), k1y = a * (-(T[0] * bz));
+        double Ux = T[0] + hh * k1x, Uy = T[1] + hh * k1y;
+        const double k2x = a * (Uy * bz), k2y = a * (-(Ux * bz));
+        Ux = T[0] + hh * k2x; Uy = T[1] + hh * k2y;
+        const double k3x = a * (Uy * bz), k3y = a * (-(Ux * bz));
+        Ux = T[0] + h * k3x; Uy = T[1] + h * k3y;
+        const double k4x = a * (Uy * bz), k4y = a * (-(Ux * bz));
+        rn[0] = r[0] + h * T[0] + h26 * (k1x + k2x + k3x);
+        rn[1] = r[1] + h * T[1] + h26 * (k1y + k2y + k3y);
+        rn[2] = r[2] + h * T[2];
+        Tn[0] = T[0] + h6 * (k1x + 2.0 * k2x + 2.0 * k3x + k4x);
+        Tn[1] = T[1] + h6 * (k1y + 2.0 * k2y + 2.0 * k3y + k4y);
+        Tn[2] = T[2];
+        return;
+    }
+    double B[3], k1[3], k2[3], k3[3], k4[3], q[3], U[3];
     field64(g, r[0], r[1], r[2], B);
     lorentz64(a, T, B, k1);
 #pragma unroll
@@ -117,8 +141,12 @@ __device__ __forceinline__ int lane_candidate(const Geom64 &g, const LayerDev *s
 // ascending wire id within an interval -- the order reading C11 fixes.  wire_label / wire_best (optional, per wire
 // of this event): reading C12.  rec / rec_count (optional): matched approaches in path order.
 // e: grid (axis tables, grid record); he: event whose hit tables are scored (== e except for refinement sub-grids).
-__device__ void eval_seed64(const BestArgs &A, const LayerDev *s_layer, int e, int he, uint32_t index, Eval64 &out,
-                            int32_t *wire_label, double *wire_best, ApproachRec *rec, int32_t *rec_count)
+// ELOSS = false (eloss_h == 0): p_n = p_0 - 0 * m = p_0 exactly, so a = kappa q / p_0 is formed once.  ELOSS = true: the
+// momentum of the NEXT step depends only on the in-gas count, known at the top of this step, so its division runs
+// beside this step's stages instead of ahead of them.
+template <bool UNI, bool ELOSS>
+__device__ void eval_seed64_t(const BestArgs &A, const LayerDev *s_layer, int e, int he, uint32_t index, Eval64 &out,
+                              int32_t *wire_label, double *wire_best, ApproachRec *rec, int32_t *rec_count)
 {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
@@ -142,10 +170,14 @@ __device__ void eval_seed64(const BestArgs &A, const LayerDev *s_layer, int e, i
     int kc = 0, w = -1;
     float wr[5] = {0.f, 0.f, 0.f, 0.f, 1.f};
     double g0 = 0.0, drift_w = 0.0;
-    double a = A.kq / p, p_of_a = p;
+    double a = A.kq / p;                                                // a = kappa q / p_n (C5/C6)
     while (n < A.max_steps) {
-        if (p != p_of_a) { a = A.kq / p; p_of_a = p; }                  // a = kappa q / p_n (C5/C6)
         double rn[3], Tn[3];
+        double p_next = p, a_next = a;
+        if (ELOSS) {                                                    // C6: p_{n+1} = p_0 - eloss_h m_{n+1}
+            p_next = p0 - A.eloss_h * (double)(m + (cn ? 1 : 0));
+            a_next = A.kq / p_next;
+        }
         // every K64 steps: this lane's candidate wire around r_n and g at r_n.  A wire outside the 3 x 3 set is at
         // least 1.5 layer pitches / 1.5 cells away, so the set stays a superset of the wires that can own a match for
         // K64 intervals (reading C8); g is carried from vertex to vertex (same operands, same value as a fresh
@@ -164,7 +196,7 @@ __device__ void eval_seed64(const BestArgs &A, const LayerDev *s_layer, int e, i
             }
         }
         kc -= 1;
-        rkn_step64(A.g, a, A.h, r, T, rn, Tn);
+        rkn_step64<UNI>(A.g, a, A.h, r, T, rn, Tn);
         double g1 = 0.0;
         if (w >= 0) {
             double d1[3], tp;
@@ -213,7 +245,7 @@ __device__ void eval_seed64(const BestArgs &A, const LayerDev *s_layer, int e, i
 #pragma unroll
         for (int i = 0; i < 3; ++i) { r[i] = rn[i]; T[i] = Tn[i]; }
         n += 1;
-        p = p0 - A.eloss_h * (double)m;                                 // C6
+        p = p_next; a = a_next;
         const bool cnext = r[0] * r[0] + r[1] * r[1] >= A.g.R0 * A.g.R0;
         if (!cn && cnext) turn += 1;                                    // C7
         cn = cnext;
@@ -225,6 +257,17 @@ __device__ void eval_seed64(const BestArgs &A, const LayerDev *s_layer, int e, i
     }
     out.n_match = n_match; out.chi2 = chi2; out.n_steps = n; out.turns = turn; out.m_gas = m;
     if (rec_count && lane == 0) *rec_count = n_rec;
+}
+
+__device__ __forceinline__ void eval_seed64(const BestArgs &A, const LayerDev *s_layer, int e, int he, uint32_t index,
+                                            Eval64 &out, int32_t *wire_label, double *wire_best, ApproachRec *rec,
+                                            int32_t *rec_count)
+{
+    const bool uni = A.g.field_kind == 0, el = A.eloss_h != 0.0;
+    if (uni && !el) eval_seed64_t<true, false>(A, s_layer, e, he, index, out, wire_label, wire_best, rec, rec_count);
+    else if (uni) eval_seed64_t<true, true>(A, s_layer, e, he, index, out, wire_label, wire_best, rec, rec_count);
+    else if (!el) eval_seed64_t<false, false>(A, s_layer, e, he, index, out, wire_label, wire_best, rec, rec_count);
+    else eval_seed64_t<false, true>(A, s_layer, e, he, index, out, wire_label, wire_best, rec, rec_count);
 }
 
 __device__ __forceinline__ void load_layers(const Geom64 &g, LayerDev *s_layer)
