@@ -1,0 +1,117 @@
+"""Turn-partition peeling (reading C18): pins of the plain CPU statement
+(oracle/peel.py) and GPU parity of cdc_peel_turns (-m gpu)."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import peel as OP
+from oracle import quality as Q
+from paper_1908_01949_b200 import synth
+
+HALF_WIDTH = [0.01, 26.0, 2.5, 2.5, 1.7]        # PAPER.md:51 (0.01 rad, 2.5 MeV) and :83 (2.6 cm, 1.7 MeV)
+
+
+def _two_turn_event(**kw):
+    cfg = synth.CONFIGS[1]
+    geom = synth.make_geometry(); field = synth.make_uniform_field()
+    ev = synth.generate_events(cfg, geom, field, 1, **kw)[0]
+    return cfg, geom, field, ev
+
+
+def test_next_entrance_is_one_helix_period_later_in_a_uniform_field():
+    # closed form: without energy loss the (x, y) projection in a uniform field is a closed circle, so the next
+    # outward crossing of rho = R0 is the seed's own (x, y) and direction, one period later:
+    # z advances by 2 pi p_z / (kappa |q| B).  The chord / lerp of the crossing are exact to the sagitta
+    # h^2 / (8 R) ~ 1.5e-3 mm and to theta^2 / 8 ~ 5e-6 in direction.
+    cfg, geom, field, ev = _two_turn_event()
+    params = dict(h=cfg.h_mm, max_steps=cfg.max_steps, window=cfg.window_mm)
+    th, z0, px, py, pz = ev.seed
+    nx = OP.next_entrance(geom, field, params, ev.seed, 3000)
+    assert nx is not None
+    x0, y0 = geom.R0_mm * math.cos(th), geom.R0_mm * math.sin(th)
+    dz = 2.0 * math.pi * pz / (0.299792458 * 1.0)
+    assert abs(nx[0] - x0) < 3e-3 and abs(nx[1] - y0) < 3e-3
+    assert abs(math.hypot(nx[0], nx[1]) - geom.R0_mm) < 1e-9            # on the cylinder
+    assert abs(nx[2] - (z0 + dz)) < 3e-3
+    p = math.sqrt(px * px + py * py + pz * pz)
+    assert abs(nx[3] - px) < 1e-5 * p and abs(nx[4] - py) < 1e-5 * p and abs(nx[5] - pz) < 1e-5 * p
+    assert abs(math.sqrt(nx[3] ** 2 + nx[4] ** 2 + nx[5] ** 2) - p) < 1e-9 * p
+
+
+def test_next_entrance_lies_on_the_chord_of_the_c_oracles_trajectory_and_loses_the_gas_energy():
+    # the Python loop of next_entrance against the C oracle's own vertices (orc_eval_seed trajectory): the crossing
+    # interval is the first (rho_n < R0 <= rho_{n+1}) after the start, the point lies on that chord at rho = R0, and
+    # with energy loss |p| = p0 - eloss * h * (vertices with rho >= R0 before it, the start counted in)  (C6)
+    cfg = synth.CONFIGS[2]
+    geom = synth.make_geometry(); field = synth.make_uniform_field()
+    ev = synth.generate_events(cfg, geom, field, 1)[0]
+    params = dict(h=cfg.h_mm, max_steps=cfg.max_steps, window=cfg.window_mm, eloss=cfg.eloss_MeV_per_mm)
+    bound = oracle.Bound(geom, field, params)
+    traj = oracle.eval_seed(bound, ev.wire_id, ev.drift_mm, ev.seed, trajectory=True)["traj"]
+    rho2 = traj[:, 0] ** 2 + traj[:, 1] ** 2
+    inside = rho2 >= geom.R0_mm ** 2
+    inside[0] = True                                                       # reading C7: the seed is in the gas
+    n = int(np.nonzero(~inside[:-1] & inside[1:])[0][0])
+    nx = OP.next_entrance(geom, field, params, ev.seed, 3000)
+    a, b = traj[n, :3], traj[n + 1, :3]
+    pos = np.array(nx[:3])
+    tau = np.dot(pos - a, b - a) / np.dot(b - a, b - a)
+    assert 0.0 <= tau <= 1.0
+    assert np.abs(a + tau * (b - a) - pos).max() < 1e-9
+    assert abs(math.hypot(nx[0], nx[1]) - geom.R0_mm) < 1e-9
+    p0 = math.sqrt(sum(float(v) ** 2 for v in ev.seed[2:]))
+    m_gas = int(inside[:n + 1].sum())
+    pn = math.sqrt(nx[3] ** 2 + nx[4] ** 2 + nx[5] ** 2)
+    assert abs(pn - (p0 - cfg.eloss_MeV_per_mm * cfg.h_mm * m_gas)) < 1e-9
+    u = np.array(nx[3:]) / pn                                              # direction between T_n and T_{n+1}
+    assert np.dot(u, traj[n, 3:]) > 1 - 1e-4 and np.dot(u, traj[n + 1, 3:]) > 1 - 1e-4
+
+
+def test_centred_grid_nodes():
+    g = OP.centred_grid([1.0, 2.0, 3.0, 4.0, 5.0], [0.5, 1.0, 0.0, 2.0, 4.0], [3, 5, 1, 2, 9])
+    nodes = [[g.lo[a] + i * g.step[a] for i in range(int(g.n[a]))] for a in range(5)]
+    assert nodes[0] == [0.5, 1.0, 1.5] and nodes[1] == [1.0, 1.5, 2.0, 2.5, 3.0]
+    assert nodes[2] == [3.0] and nodes[3] == [2.0, 6.0] and nodes[4][0] == 1.0 and nodes[4][4] == 5.0 and nodes[4][8] == 9.0
+    assert g.n_seeds == 3 * 5 * 2 * 9
+
+
+def test_peeling_a_smear_free_noise_free_event_returns_the_truth_partitions():
+    # every signal hit of a two-turn event ends in the partition of its truth turn, nothing is left, the loop stops
+    # because fewer than min_hits hits remain: efficiency = purity = 1 for both partitions (Eq. 2, 3)
+    cfg, geom, field, ev = _two_turn_event(sigma_drift=0.0, noise=0.0)
+    params = dict(h=cfg.h_mm, max_steps=cfg.max_steps, window=cfg.window_mm)
+    grid0, _ = synth.truth_anchored_grid(ev.seed, 3)
+    r = OP.peel(geom, field, params, ev.wire_id, ev.drift_mm, grid0, [3] * 5, HALF_WIDTH, max_partitions=4,
+                min_hits=10, min_classified=5, n_proc=4)
+    assert r["status"] == 1 and r["seeds"].shape == (2, 5)
+    q = Q.classification_quality(r["partition"], ev.truth_turn, 2)
+    assert q["efficiency"].tolist() == [1.0, 1.0] and q["purity"].tolist() == [1.0, 1.0]
+    assert np.array_equal(r["partition"], ev.truth_turn)
+    assert np.abs(r["seeds"][0] - ev.seed).max() == 0.0                    # the truth is a node of the first grid
+    # the second partition's seed is one helix period after the first (uniform field, no loss)
+    dz = 2.0 * math.pi * ev.seed[4] / 0.299792458
+    assert abs(r["seeds"][1][1] - (ev.seed[1] + dz)) <= 26.0
+    assert r["n_match"].sum() >= int((ev.truth_turn >= 0).sum())
+
+
+def test_peeling_stops_for_each_listed_reason():
+    cfg, geom, field, ev = _two_turn_event()
+    params = dict(h=cfg.h_mm, max_steps=cfg.max_steps, window=cfg.window_mm)
+    grid0, _ = synth.truth_anchored_grid(ev.seed, 3)
+    kw = dict(n_proc=4)
+    r = OP.peel(geom, field, params, ev.wire_id, ev.drift_mm, grid0, [1] * 5, HALF_WIDTH, max_partitions=1, **kw)
+    assert r["status"] == 3 and r["seeds"].shape[0] == 1 and set(np.unique(r["partition"])) <= {-1, 0}
+    r = OP.peel(geom, field, params, ev.wire_id, ev.drift_mm, grid0, [1] * 5, HALF_WIDTH, min_hits=10 ** 6, **kw)
+    assert r["status"] == 1 and r["seeds"].shape[0] == 0 and (r["partition"] == -1).all()
+    r = OP.peel(geom, field, params, ev.wire_id, ev.drift_mm, grid0, [1] * 5, HALF_WIDTH, min_classified=10 ** 6, **kw)
+    assert r["status"] == 2 and r["seeds"].shape[0] == 0 and (r["partition"] == -1).all()
+    # a track that leaves through the end plate before it comes back: |z| > 750 mm (C7)
+    far = np.array(ev.seed); far[1] = 700.0 * np.sign(ev.seed[4]); far = far.astype(np.float32).astype(np.float64)
+    gfar, _ = synth.truth_anchored_grid(far, 1)
+    r = OP.peel(geom, field, params, ev.wire_id, ev.drift_mm, gfar, [1] * 5, HALF_WIDTH, min_classified=0, **kw)
+    assert r["status"] == 4 and r["seeds"].shape[0] == 1
+    # classified hits are disjoint between partitions and never noise-free-of-charge: every label is a recorded partition
+    r = OP.peel(geom, field, params, ev.wire_id, ev.drift_mm, grid0, [3] * 5, HALF_WIDTH, max_partitions=3, **kw)
+    assert r["partition"].max() < r["seeds"].shape[0]
