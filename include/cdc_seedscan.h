@@ -216,6 +216,38 @@ int32_t cdc_classification_quality(const cdc_events *ev, int32_t n_turns, const 
 int32_t cdc_common_hits(const cdc_events *ev, const int32_t *d_labels_a, const int32_t *d_labels_b,
                         int32_t turn_a, int32_t turn_b, int32_t *d_n_common, void *stream);
 
+/* Turn-partition peeling: the event reconstruction loop of PAPER.md:83 (section 2.3, Fig. 7) without the Kalman fit
+ * (reading C18).  Per event, for partition k = 0, 1, ...:
+ *   scan the partition's grid over the still unclassified hits (cdc_seed_scan + cdc_best_track); the partition's hits
+ *   are those the best seed's track matches in its FIRST passage through the gas (turn label 0; "classified
+ *   as the hits of the turn partition being investigated"); they are removed from the event; the best seed is
+ *   extrapolated with the same fp64 RKN steps to its next outward crossing of rho = R0, and the neighbouring
+ *   partition's grid is n[] nodes per axis centred on that state, +- half_width[] (theta rad, z mm, px, py, pz MeV/c;
+ *   node i = (c - hw) + i * 2 hw / (n - 1), or c alone when n = 1).
+ * Stop reasons (h_status): 1 = fewer than min_hits unclassified hits remain (the paper: ten), 2 = the partition has
+ * fewer than min_classified hits (it is discarded), 3 = max_partitions recorded, 4 = the track ended (end plate, outer
+ * wall, extrap_max_steps, p <= 1 MeV/c) before the next entrance.  params->charge / reversed exit-side seeds make the
+ * extrapolation the paper's backward one (see cdc_common_hits).
+ * h_grids0: partition 0's grid per event.  Host outputs: h_n_partitions [E], h_status [E], h_seeds [E][P][5] (best
+ * seed values), h_n_match [E][P], h_chi2 [E][P], h_centres_or_null [E][P][5] (grid centre of partition k >= 1; row 0
+ * is zero); P = max_partitions <= 8; rows k >= h_n_partitions[e] are zero.  d_partition [total_hits] (device, upload
+ * order): partition index of every hit, or -1.  The events' hit tables are restored before the call returns.
+ * Synchronises once per partition (the host turns the extrapolated state into the next grid: atan2 and the cos / sin
+ * of the theta nodes come from the host libm, reading C11).  CDC_ERR_RANGE if a scan's candidate pool overflowed. */
+typedef struct {
+    int32_t max_partitions;   /* P, 1..8 */
+    int32_t min_hits;         /* >= 0; the paper: 10 */
+    int32_t min_classified;   /* >= 0 */
+    int32_t extrap_max_steps; /* >= 1 */
+    int32_t n[5];             /* nodes per axis of the grids of partitions 1.. (1..4096 each) */
+    int32_t pad_;
+    double half_width[5];
+} cdc_peel_params;
+int32_t cdc_peel_turns(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec *h_grids0,
+                       const cdc_scan_params *params, const cdc_peel_params *pp, int32_t *h_n_partitions,
+                       int32_t *h_status, double *h_seeds, uint32_t *h_n_match, double *h_chi2,
+                       double *h_centres_or_null, int32_t *d_partition, void *stream);
+
 /* MEASURED COMPARISON POINT, not the product path: the paper's own thread mapping (v1, PAPER.md:73,
  * Fig. 6) -- one block per seed, one thread per fired wire, every thread repeating the RKN propagation -- re-created on
  * sm_100a with the same arithmetic and scoring rule as cdc_seed_scan.  Evaluates the n_seeds seeds d_seed_index[] (linear

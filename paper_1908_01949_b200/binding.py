@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(HERE, "libcdc_seedscan.so")
 EXPORTS = ["cdc_last_error", "cdc_geometry_create", "cdc_geometry_destroy", "cdc_geometry_wire_table",
            "cdc_event_upload", "cdc_events_destroy", "cdc_events_tables", "cdc_hough_dims",
            "cdc_hough_seed_ranges", "cdc_seed_scan", "cdc_scan_get_stats", "cdc_best_track",
-           "cdc_find_tracks_host", "cdc_refine_tracks", "cdc_classification_quality", "cdc_common_hits", "cdc_seed_scan_paper_mapping", "cdc_fp32_peak_probe", "cdc_kernel_launch_count"]
+           "cdc_find_tracks_host", "cdc_refine_tracks", "cdc_peel_turns", "cdc_classification_quality", "cdc_common_hits", "cdc_seed_scan_paper_mapping", "cdc_fp32_peak_probe", "cdc_kernel_launch_count"]
 
 
 class CdcError(RuntimeError):
@@ -55,6 +55,11 @@ class HoughParams(C.Structure):
 
 class RefineParams(C.Structure):
     _fields_ = [("n_parents", C.c_int32), ("n_iterations", C.c_int32)]
+
+
+class PeelParams(C.Structure):
+    _fields_ = [("max_partitions", C.c_int32), ("min_hits", C.c_int32), ("min_classified", C.c_int32),
+                ("extrap_max_steps", C.c_int32), ("n", C.c_int32 * 5), ("pad_", C.c_int32), ("half_width", C.c_double * 5)]
 
 
 class ScanStats(C.Structure):
@@ -268,6 +273,24 @@ def cdc_refine_tracks(geometry: Geometry, events: Events, grids: C.Array, params
                                    _hp(nm), _hp(chi2), _hp(q), _hp(lab), _hp(tS), _hp(tq), _stream(stream)))
     return dict(seed=seed, S=S, n_match=nm, chi2=chi2, q=q, labels=None if lab is None else lab[:events.n_hits],
                 trace_S=tS, trace_q=tq)
+
+
+def cdc_peel_turns(geometry: Geometry, events: Events, grids0: C.Array, params: ScanParams, n: Sequence[int],
+                   half_width: Sequence[float], max_partitions: int = 4, min_hits: int = 10, min_classified: int = 5,
+                   extrap_max_steps: int = 3000, stream=None) -> dict:
+    """Turn-partition peeling.  Host (numpy) outputs; `partition` is read back from the device."""
+    import torch
+    E, P = events.n_events, int(max_partitions)
+    pp = PeelParams(P, int(min_hits), int(min_classified), int(extrap_max_steps), (C.c_int32 * 5)(*[int(v) for v in n]), 0,
+                    (C.c_double * 5)(*[float(v) for v in half_width]))
+    n_part = np.zeros(E, dtype=np.int32); status = np.zeros(E, dtype=np.int32)
+    seeds = np.zeros((E, P, 5)); nm = np.zeros((E, P), dtype=np.uint32); chi2 = np.zeros((E, P)); centres = np.zeros((E, P, 5))
+    d_part = torch.empty(max(events.n_hits, 1), dtype=torch.int32, device="cuda")
+    _check(lib().cdc_peel_turns(geometry.handle, events.handle, grids0, C.byref(params), C.byref(pp), _hp(n_part),
+                                _hp(status), _hp(seeds), _hp(nm), _hp(chi2), _hp(centres), _dp(d_part), _stream(stream)))
+    torch.cuda.synchronize()
+    return dict(n_partitions=n_part, status=status, seeds=seeds, n_match=nm, chi2=chi2, centres=centres,
+                partition=d_part[:events.n_hits].cpu().numpy(), d_partition=d_part)
 
 
 def cdc_classification_quality(events: Events, n_turns: int, d_labels, d_truth, stream=None) -> dict:

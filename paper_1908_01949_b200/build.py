@@ -1,5 +1,5 @@
 """Build paper_1908_01949_b200/libcdc_seedscan.so (the C-ABI library of include/cdc_seedscan.h) with nvcc
-for sm_100a, in-tree.  best.cu is compiled with -fmad=false (IEEE fp64 without contraction, C11)."""
+for sm_100a, in-tree.  best.cu, refine.cu and peel.cu are compiled with -fmad=false (IEEE fp64 without contraction, C11)."""
 import os
 import subprocess
 import sys
@@ -15,8 +15,9 @@ SOURCES = {                      # file -> extra flags
     "abi.cu": [], "abi_events.cu": [], "abi_scan.cu": [], "abi_e2e.cu": [],
     "events.cu": [], "hough.cu": [], "scan.cu": ["-Xptxas", "-v"], "peak.cu": [],
     "best.cu": ["-fmad=false"], "refine.cu": ["-fmad=false"], "abi_refine.cu": [], "quality.cu": [], "paper_v1.cu": [],
+    "peel.cu": ["-fmad=false"], "abi_peel.cu": [],
 }
-HEADERS = [os.path.join(CSRC, "cdc_internal.cuh"), os.path.join(CSRC, "eval64.cuh"), os.path.join(CSRC, "scan_common.cuh"), os.path.join(HERE, "..", "include", "cdc_seedscan.h")]
+HEADERS = [os.path.join(CSRC, "peel.cuh"), os.path.join(CSRC, "refine.cuh"), os.path.join(CSRC, "cdc_internal.cuh"), os.path.join(CSRC, "eval64.cuh"), os.path.join(CSRC, "scan_common.cuh"), os.path.join(HERE, "..", "include", "cdc_seedscan.h")]
 
 
 def _stale(target, deps):

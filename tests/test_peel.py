@@ -115,3 +115,77 @@ def test_peeling_stops_for_each_listed_reason():
     # classified hits are disjoint between partitions and never noise-free-of-charge: every label is a recorded partition
     r = OP.peel(geom, field, params, ev.wire_id, ev.drift_mm, grid0, [3] * 5, HALF_WIDTH, max_partitions=3, **kw)
     assert r["partition"].max() < r["seeds"].shape[0]
+
+
+def _gpu_vs_oracle(cfg_id, n_events, n0, n, max_steps, P=3, **gen_kw):
+    from paper_1908_01949_b200 import api, binding as B
+    cfg = synth.CONFIGS[cfg_id]
+    geom = synth.make_geometry()
+    field = synth.make_uniform_field() if cfg.field_kind == 0 else synth.make_table_field()
+    events = synth.generate_events(cfg, geom, field, n_events, **gen_kw)
+    grids = [synth.truth_anchored_grid(ev.seed, n0)[0] for ev in events]
+    sc = api.SeedScanner(geom, field)
+    off, w, d = synth.pack_hits(events)
+    E = sc.upload(off, w, d)
+    bits_before = E.tables()[1].copy()
+    params = dict(h=cfg.h_mm, max_steps=max_steps, window=cfg.window_mm, eloss=cfg.eloss_MeV_per_mm)
+    Pg = B.scan_params(cfg.h_mm, max_steps, cfg.window_mm, cfg.eloss_MeV_per_mm)
+    out = B.cdc_peel_turns(sc.geometry, E, B.grid_specs(grids), Pg, n, HALF_WIDTH, max_partitions=P, min_hits=10,
+                           min_classified=5, extrap_max_steps=3000)
+    assert np.array_equal(E.tables()[1], bits_before)                       # the events are handed back unchanged
+    res = []
+    for e, (ev, g0) in enumerate(zip(events, grids)):
+        r = OP.peel(geom, field, params, ev.wire_id, ev.drift_mm, g0, n, HALF_WIDTH, max_partitions=P, min_hits=10,
+                    min_classified=5, extrap_max_steps=3000)
+        k = r["seeds"].shape[0]
+        assert out["status"][e] == r["status"] and out["n_partitions"][e] == k, (e, out["status"][e], r["status"])
+        assert np.array_equal(out["partition"][off[e]:off[e + 1]], r["partition"]), e       # bit-exact labels
+        assert np.array_equal(out["seeds"][e, :k], r["seeds"]), e                           # seeds as doubles
+        assert np.array_equal(out["n_match"][e, :k].astype(np.int64), r["n_match"]), e
+        assert np.array_equal(out["chi2"][e, :k], r["chi2"]), e
+        assert np.array_equal(out["centres"][e, 1:1 + r["centres"].shape[0]], r["centres"]), e   # extrapolation, fp64
+        assert not out["seeds"][e, k:].any()
+        res.append((ev, r))
+    sc.close()
+    return res
+
+
+@pytest.mark.gpu
+def test_gpu_peeling_equals_oracle_two_turn_events_uniform_field():
+    res = _gpu_vs_oracle(1, 3, 6, [5, 5, 5, 5, 5], 1500)
+    # the method works on these events: both partitions found, most of their hits in the right one
+    for ev, r in res:
+        assert r["seeds"].shape[0] >= 2
+        q = Q.classification_quality(r["partition"], ev.truth_turn, 2)
+        assert q["efficiency"].min() > 0.5 and q["purity"].min() > 0.6
+
+
+@pytest.mark.gpu
+def test_gpu_peeling_equals_oracle_with_energy_loss_three_turns():
+    _gpu_vs_oracle(2, 1, 6, [5, 5, 5, 5, 5], 1500, P=4)
+
+
+@pytest.mark.gpu
+def test_gpu_peeling_equals_oracle_table_field_mixed_turn_counts():
+    _gpu_vs_oracle(3, 4, 5, [4, 4, 4, 4, 4], 1500)
+
+
+@pytest.mark.gpu
+def test_gpu_peeling_rejects_bad_arguments():
+    from paper_1908_01949_b200 import api, binding as B
+    cfg, geom, field, ev = _two_turn_event()
+    sc = api.SeedScanner(geom, field)
+    off, w, d = synth.pack_hits([ev])
+    E = sc.upload(off, w, d)
+    g = B.grid_specs([synth.truth_anchored_grid(ev.seed, 2)[0]])
+    Pg = B.scan_params(cfg.h_mm, 500, cfg.window_mm)
+    for kw in (dict(max_partitions=0), dict(max_partitions=9), dict(min_hits=-1), dict(extrap_max_steps=0)):
+        with pytest.raises(B.CdcError):
+            B.cdc_peel_turns(sc.geometry, E, g, Pg, [2] * 5, HALF_WIDTH, **kw)
+    with pytest.raises(B.CdcError):
+        B.cdc_peel_turns(sc.geometry, E, g, Pg, [0, 2, 2, 2, 2], HALF_WIDTH)
+    with pytest.raises(B.CdcError):
+        B.cdc_peel_turns(sc.geometry, E, g, Pg, [2] * 5, [0.01, -1.0, 1, 1, 1])
+    out = B.cdc_peel_turns(sc.geometry, E, g, Pg, [2] * 5, HALF_WIDTH, min_hits=10 ** 6)      # nothing to do
+    assert out["status"].tolist() == [1] and out["n_partitions"].tolist() == [0] and (out["partition"] == -1).all()
+    sc.close()
