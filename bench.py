@@ -61,6 +61,9 @@ def parse():
     ap.add_argument("--paper-mapping", action="store_true",
                     help="measure the re-created thread mapping of the paper (one block per seed, one thread per fired "
                          "wire) against the product kernel on a sample of the workload's seeds (comparison point)")
+    ap.add_argument("--peel", action="store_true",
+                    help="measure the turn-partition peeling loop (cdc_peel_turns, SURVEY 8(f) #3) on the workload's "
+                         "events: events/s, partitions found, efficiency / purity against the synthetic truth")
     return ap.parse_args()
 
 
@@ -374,9 +377,53 @@ def run_paper_mapping(args):
                       "product_kernel_seeds_per_s": ours, "ratio": ours / (n / t_v1)}))
 
 
+def run_peel(args):
+    """the event reconstruction loop without the fit.  Partition 0's grid is the workload's own;
+    the following partitions use 8^5 nodes centred on the extrapolated seed with the paper's quoted resolutions as
+    half-widths.  One partition's track is at most max_steps / n_turns steps long."""
+    import torch
+    from oracle import quality as Q          # Eq. (2), (3) on the host: reporting only, not part of the timed path
+    from paper_1908_01949_b200 import api, binding as B
+    torch.cuda.set_device(0)
+    cfg_id, cfg, geom, field, events, grids = make_workload(args, 0)
+    sc = api.SeedScanner(geom, field)
+    off, w, d = synth.pack_hits(events)
+    ev = B.Events(sc.geometry, off, w, d)
+    steps = 1500
+    P = B.scan_params(cfg.h_mm, steps, cfg.window_mm, cfg.eloss_MeV_per_mm)
+    hw = [0.01, 26.0, 2.5, 2.5, 1.7]
+    ms = []
+    n0 = B.cdc_kernel_launch_count()
+    for it in range(args.warmup + args.steps):
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); e0.record()
+        out = B.cdc_peel_turns(sc.geometry, ev, B.grid_specs(grids), P, [8] * 5, hw, max_partitions=4)
+        e1.record(); e1.synchronize()
+        if it == args.warmup - 1:
+            n0 = B.cdc_kernel_launch_count()
+        if it >= args.warmup:
+            ms.append(e0.elapsed_time(e1))
+    launches = (B.cdc_kernel_launch_count() - n0) // max(args.steps, 1)
+    eff, pur, found = [], [], 0
+    for e, evt in enumerate(events):
+        q = Q.classification_quality(out["partition"][off[e]:off[e + 1]], evt.truth_turn, evt.n_turns)
+        eff += [float(v) for v in q["efficiency"] if v >= 0]; pur += [float(v) for v in q["purity"] if v >= 0]
+        found += int(out["n_partitions"][e] >= evt.n_turns)
+    t = float(np.mean(ms)) * 1e-3
+    print(json.dumps({"measurement": "turn_peeling", "workload": args.workload, "events": len(events),
+                      "seeds_partition0": int(grids[0].n_seeds), "seeds_next": 8 ** 5, "max_steps": steps,
+                      "ms_per_call": t * 1e3, "events_per_s": len(events) / t, "kernel_launches_per_call": int(launches),
+                      "partitions_found": [int(v) for v in out["n_partitions"]], "true_turns": [e.n_turns for e in events],
+                      "status": [int(v) for v in out["status"]], "events_with_all_turns": found,
+                      "mean_efficiency": float(np.mean(eff)) if eff else None,
+                      "mean_purity": float(np.mean(pur)) if pur else None}))
+
+
 if __name__ == "__main__":
     a = parse()
-    if a.paper_mapping:
+    if a.peel:
+        run_peel(a)
+    elif a.paper_mapping:
         run_paper_mapping(a)
     elif a.sweep:
         run_sweep(a)
