@@ -366,15 +366,25 @@ def run_paper_mapping(args):
         e1.record(); e1.synchronize()
         if it:
             ms.append(e0.elapsed_time(e1))
+    ms2 = []
+    for it in range(3):                      # the two-kernel mapping: record, then DCA per wire
+        k = B.cdc_seed_scan_paper_mapping_v2(sc.geometry, ev, 0, grids[0], P, d_sel, d_nm, d_c2, timed=True)
+        if it:
+            ms2.append(k)
     d_key = torch.zeros(len(events), dtype=torch.int64, device="cuda")
     for it in range(3):
         B.cdc_seed_scan(sc.geometry, ev, B.grid_specs(grids), P, d_key)
         st = B.cdc_scan_get_stats(ev)
     t_v1 = float(np.mean(ms)) * 1e-3
+    k1, k2 = (float(v) * 1e-3 for v in np.mean(ms2, axis=0))
     ours = st["n_seeds"] / (st["kernel_ms"] * 1e-3)
     print(json.dumps({"comparison": "paper_v1_mapping", "workload": args.workload, "hits": int(off[1]), "sample_seeds": n,
                       "paper_mapping_ms": t_v1 * 1e3, "paper_mapping_seeds_per_s": n / t_v1,
                       "product_kernel_seeds_per_s": ours, "ratio": ours / (n / t_v1)}))
+    print(json.dumps({"comparison": "paper_v2_mapping", "workload": args.workload, "hits": int(off[1]), "sample_seeds": n,
+                      "record_kernel_ms": k1 * 1e3, "dca_kernel_ms": k2 * 1e3, "record_bytes": 32 * n * (cfg.max_steps + 1),
+                      "paper_mapping_seeds_per_s": n / (k1 + k2), "product_kernel_seeds_per_s": ours,
+                      "ratio": ours / (n / (k1 + k2))}))
 
 
 def run_peel(args):

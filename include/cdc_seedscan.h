@@ -257,6 +257,16 @@ int32_t cdc_seed_scan_paper_mapping(const cdc_geometry *g, cdc_events *ev, int32
                                     const cdc_scan_params *params, const int64_t *d_seed_index, int32_t n_seeds,
                                     uint32_t *d_n_match, float *d_chi2, void *stream);
 
+/* MEASURED COMPARISON POINT, not the product path: the paper's second mapping ("kernel function
+ * separation").  Kernel 1: one thread per seed propagates it and records every vertex (32 bytes x
+ * n_seeds x (max_steps + 1) of device memory, CDC_ERR_RANGE above 16 GiB); kernel 2: one block per seed, one thread per
+ * fired wire, walks the record and takes the approaches between recorded vertices.  Same arguments and outputs as
+ * cdc_seed_scan_paper_mapping, bit-equal results; h_ms2_or_null (host, 2 doubles): device time of the two kernels in
+ * ms (the call then synchronises).  No energy loss. */
+int32_t cdc_seed_scan_paper_mapping_v2(const cdc_geometry *g, cdc_events *ev, int32_t event, const cdc_grid_spec *h_grid,
+                                       const cdc_scan_params *params, const int64_t *d_seed_index, int32_t n_seeds,
+                                       uint32_t *d_n_match, float *d_chi2, double *h_ms2_or_null, void *stream);
+
 /* Number of kernels this library has launched in this process so far (bench.py's gpu_launches). */
 uint64_t cdc_kernel_launch_count(void);
 

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(HERE, "libcdc_seedscan.so")
 EXPORTS = ["cdc_last_error", "cdc_geometry_create", "cdc_geometry_destroy", "cdc_geometry_wire_table",
            "cdc_event_upload", "cdc_events_destroy", "cdc_events_tables", "cdc_hough_dims",
            "cdc_hough_seed_ranges", "cdc_seed_scan", "cdc_scan_get_stats", "cdc_best_track",
-           "cdc_find_tracks_host", "cdc_refine_tracks", "cdc_peel_turns", "cdc_classification_quality", "cdc_common_hits", "cdc_seed_scan_paper_mapping", "cdc_fp32_peak_probe", "cdc_kernel_launch_count"]
+           "cdc_find_tracks_host", "cdc_refine_tracks", "cdc_peel_turns", "cdc_classification_quality", "cdc_common_hits", "cdc_seed_scan_paper_mapping", "cdc_seed_scan_paper_mapping_v2", "cdc_fp32_peak_probe", "cdc_kernel_launch_count"]
 
 
 class CdcError(RuntimeError):
@@ -322,6 +322,17 @@ def cdc_seed_scan_paper_mapping(geometry: Geometry, events: Events, event: int, 
     _check(lib().cdc_seed_scan_paper_mapping(geometry.handle, events.handle, C.c_int32(event), grid_specs([grid]),
                                              C.byref(params), _dp(d_seed_index), C.c_int32(int(d_seed_index.numel())),
                                              _dp(d_n_match), _dp(d_chi2), _stream(stream)))
+
+
+def cdc_seed_scan_paper_mapping_v2(geometry: Geometry, events: Events, event: int, grid, params: ScanParams, d_seed_index,
+                                   d_n_match, d_chi2, timed: bool = False, stream=None):
+    """The paper's two-kernel mapping (record all steps, then DCA per wire; comparison point only).
+    timed=True returns the device times (ms) of the two kernels."""
+    ms = np.zeros(2) if timed else None
+    _check(lib().cdc_seed_scan_paper_mapping_v2(geometry.handle, events.handle, C.c_int32(event), grid_specs([grid]),
+                                                C.byref(params), _dp(d_seed_index), C.c_int32(int(d_seed_index.numel())),
+                                                _dp(d_n_match), _dp(d_chi2), _hp(ms), _stream(stream)))
+    return ms
 
 
 def cdc_kernel_launch_count() -> int:

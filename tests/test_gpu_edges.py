@@ -201,6 +201,16 @@ def test_paper_thread_mapping_gives_the_same_scores(cfg_id):
     for i in np.nonzero(nm != orc["n_match"])[0]:
         assert U.explain_mismatch(bound, events[1], grids[1].node(grids[1].unravel(int(sel[i]))), cfg, geom)
     assert (nm != orc["n_match"]).sum() <= 2
+    # the two-kernel mapping (record every step, then DCA per wire from the record): same arithmetic,
+    # so bit-equal to the one-kernel mapping
+    d_nm2 = torch.zeros_like(d_nm); d_c22 = torch.zeros_like(d_c2)
+    ms = B.cdc_seed_scan_paper_mapping_v2(sc.geometry, E, 1, grids[1], P, d_sel, d_nm2, d_c22, timed=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(d_nm2.cpu().numpy(), nm) and ms[0] > 0 and ms[1] > 0
+    assert np.allclose(d_c22.cpu().numpy(), c2, rtol=1e-5, atol=1e-6)       # block-level float atomics: order differs
+    with pytest.raises(B.CdcError):                                         # 32 B x seeds x steps beyond 16 GiB
+        B.cdc_seed_scan_paper_mapping_v2(sc.geometry, E, 1, grids[1], B.scan_params(cfg.h_mm, 2_000_000, cfg.window_mm),
+                                         d_sel, d_nm2, d_c22)
 
 
 def test_tightly_curling_seeds_use_the_short_lookup_cadence(setup):
