@@ -392,7 +392,6 @@ def run_peel(args):
     the following partitions use 8^5 nodes centred on the extrapolated seed with the paper's quoted resolutions as
     half-widths.  One partition's track is at most max_steps / n_turns steps long."""
     import torch
-    from oracle import quality as Q          # Eq. (2), (3) on the host: reporting only, not part of the timed path
     from paper_1908_01949_b200 import api, binding as B
     torch.cuda.set_device(0)
     cfg_id, cfg, geom, field, events, grids = make_workload(args, 0)
@@ -414,10 +413,13 @@ def run_peel(args):
         if it >= args.warmup:
             ms.append(e0.elapsed_time(e1))
     launches = (B.cdc_kernel_launch_count() - n0) // max(args.steps, 1)
+    # Eq. (2), (3) against the generator's truth turns, by the library's own kernel (not part of the timed region)
+    truth = torch.tensor(np.concatenate([e.truth_turn for e in events]).astype(np.int32), device="cuda")
+    q = B.cdc_classification_quality(ev, 3, out["d_partition"], truth)
     eff, pur, found = [], [], 0
     for e, evt in enumerate(events):
-        q = Q.classification_quality(out["partition"][off[e]:off[e + 1]], evt.truth_turn, evt.n_turns)
-        eff += [float(v) for v in q["efficiency"] if v >= 0]; pur += [float(v) for v in q["purity"] if v >= 0]
+        eff += [float(v) for v in q["efficiency"][e][:evt.n_turns] if v >= 0]
+        pur += [float(v) for v in q["purity"][e][:evt.n_turns] if v >= 0]
         found += int(out["n_partitions"][e] >= evt.n_turns)
     t = float(np.mean(ms)) * 1e-3
     print(json.dumps({"measurement": "turn_peeling", "workload": args.workload, "events": len(events),

@@ -66,7 +66,7 @@ __device__ __forceinline__ void slot_push(Slots &S, int w, float g)
 
 struct LookupCtx {         // the vertex a lookup is made from
     float x, xl, y, yl, z, Tx, Ty, Tz;     // the vertex itself: g of a new slot is evaluated here
-    float cz, phi, g_dead;                 // height and azimuth of the lookup centre
+    float cz, phi, g_dead, g_far;          // height and azimuth of the lookup centre
 };
 
 // a candidate with a hit becomes a live slot unless the track has already passed it for good: once g exceeds
@@ -78,7 +78,7 @@ __device__ __forceinline__ void consider(const ScanArgs &A, const uint32_t *s_bi
     float ex, ey, eu;
     cnt += 1u;
     const float g = wire_g(__ldg(A.gd.wire4 + w), A.uz, A.inv_uz, V.x, V.xl, V.y, V.yl, V.z, V.Tx, V.Ty, V.Tz, ex, ey, eu);
-    if (g <= V.g_dead) slot_push(S, w, g);
+    if (g <= V.g_dead && g > V.g_far) slot_push(S, w, g);
 }
 
 // cells kc and its nearer neighbour of layer j around azimuth phi at height z -> push those with a hit
@@ -233,6 +233,9 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
                 {
                     const float cbend = (ELOSS ? 1.05f : 1.0f) * A.delta_max * fabsf(a) * A.b_max;
                     V.g_dead = fmaf(A.hold_path * 0.25f, cbend * cbend, 0.02f);
+                    // nor can a wire own an approach before the next lookup if g is still far below zero: g grows by at
+                    // most h (1 + |delta| |a| B) per step (g' = 1 - (T.u)^2 + delta . T')
+                    V.g_far = -fmaf((float)kcount * h, 1.0f + cbend, 0.25f);
                 }
                 lookup_layer(A, s_layer, s_bits, jc, V, S, cnt);
                 lookup_layer(A, s_layer, s_bits, j2, V, S, cnt);
