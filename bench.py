@@ -271,6 +271,7 @@ def run_ours(args):
                 "rkn_steps_per_s": steps_all / (total_ms * 1e-3), "events_per_s": events_all * K / (total_ms * 1e-3),
                 "scan_kernel_ms": sum(kernel_ms) / K, "scan_kernel_share": ksum_ms / total_ms,
                 "rkn_steps_per_s_kernel": acc["n_steps"] / k_s,
+                "candidate_pool": {"entries_per_step": acc["n_pool"] / K, "capacity": int(st["pool_cap"])},
                 "clocks": clocks,
                 "e2e": {"value": seeds_all * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
                 "gpu_launches": int(launches),

@@ -16,10 +16,14 @@ struct Scratch {                       // device buffers of one call, freed on e
     int64_t *seed = nullptr;
     uint32_t *nmatch = nullptr;
     cdc_events *ev = nullptr;
-    ~Scratch()
+    cudaStream_t s = nullptr;
+    template <typename T>
+    cudaError_t get(T **p, size_t n) { return cudaMallocAsync((void **)p, sizeof(T) * n, s); }   // stream-ordered pool:
+    ~Scratch()                                                                                  // no device sync
     {
-        cudaFree(zref); cudaFree(ranges); cudaFree(chi2); cudaFree(peak); cudaFree(labels); cudaFree(key);
-        cudaFree(seed); cudaFree(nmatch);
+        void *all[] = {zref, ranges, chi2, peak, labels, key, seed, nmatch};
+        for (void *p : all)
+            if (p) cudaFreeAsync(p, s);
         if (ev) cdc_events_destroy(ev);
     }
 };
@@ -38,19 +42,20 @@ extern "C" int32_t cdc_find_tracks_host(const cdc_geometry *g, int32_t n_events,
     if (hp && !h_zref_mm) CDC_FAIL(CDC_ERR_INVALID, "cdc_find_tracks_host: Hough ranges need h_zref_mm");
     cudaStream_t s = (cudaStream_t)stream;
     Scratch S;
+    S.s = s;
     int32_t rc = cdc_event_upload(g, n_events, h_hit_offsets, h_wire_id, h_drift_mm, 0, stream, &S.ev);
     if (rc != CDC_OK) return rc;
     const size_t E = (size_t)n_events, H = std::max<size_t>((size_t)h_hit_offsets[n_events], 1);
-    CDC_CUDA(cudaMalloc((void **)&S.key, sizeof(uint64_t) * E));
-    CDC_CUDA(cudaMalloc((void **)&S.seed, sizeof(int64_t) * E));
-    CDC_CUDA(cudaMalloc((void **)&S.nmatch, sizeof(uint32_t) * E));
-    CDC_CUDA(cudaMalloc((void **)&S.chi2, sizeof(double) * E));
-    CDC_CUDA(cudaMalloc((void **)&S.labels, sizeof(int32_t) * H));
+    CDC_CUDA(S.get(&S.key, E));
+    CDC_CUDA(S.get(&S.seed, E));
+    CDC_CUDA(S.get(&S.nmatch, E));
+    CDC_CUDA(S.get(&S.chi2, E));
+    CDC_CUDA(S.get(&S.labels, H));
     std::vector<cdc_grid_spec> grids(h_grids, h_grids + n_events);
     if (hp) {
-        CDC_CUDA(cudaMalloc((void **)&S.zref, sizeof(float) * E));
-        CDC_CUDA(cudaMalloc((void **)&S.ranges, sizeof(double) * 6 * E));
-        CDC_CUDA(cudaMalloc((void **)&S.peak, sizeof(int32_t) * 4 * E));
+        CDC_CUDA(S.get(&S.zref, E));
+        CDC_CUDA(S.get(&S.ranges, 6 * E));
+        CDC_CUDA(S.get(&S.peak, 4 * E));
         CDC_CUDA(cudaMemcpyAsync(S.zref, h_zref_mm, sizeof(float) * E, cudaMemcpyHostToDevice, s));
         rc = cdc_hough_seed_ranges(g, S.ev, hp, params->charge, S.zref, S.ranges, S.peak, nullptr, stream);
         if (rc != CDC_OK) return rc;

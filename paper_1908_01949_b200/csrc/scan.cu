@@ -358,7 +358,9 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
     }
     run = __shfl_sync(0xffffffffu, run, 0);
     const float S_run = __uint_as_float((uint32_t)(run >> 32));
-    const bool cand = valid && (Sc >= S_run - A.margin);
+    // a seed without any match (S = 0 exactly) cannot beat index 0, which ties with it and wins on the index: only
+    // index 0 stands in for all of them, so an event (or a neighbourhood) without hits cannot flood the pool
+    const bool cand = valid && (Sc >= S_run - A.margin) && (Sc > 0.0f || index == 0u);
     const unsigned ballot = __ballot_sync(0xffffffffu, cand);
     if (ballot) {
         unsigned base = 0;

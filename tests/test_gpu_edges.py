@@ -90,6 +90,20 @@ def test_empty_event_and_ragged_grid(setup):
     assert gpu["labels"].size == ev.wire_id.size
 
 
+def test_event_without_hits_on_a_grid_larger_than_the_candidate_pool(setup):
+    """Every seed of an event without hits scores S = 0: the tie goes to index 0 and the 65 536-entry candidate pool
+    must not overflow (only index 0 stands in for the seeds without a match)."""
+    cfg, geom, field, events, grids, sc = setup
+    ev = events[0]
+    g_big = synth.truth_anchored_grid(ev.seed, 12)[0]                    # 248 832 seeds
+    off = np.array([0, 0, ev.wire_id.size], dtype=np.int32)
+    E = sc.upload(off, ev.wire_id, ev.drift_mm)
+    gpu = sc.scan(E, [g_big, g_big], B.scan_params(cfg.h_mm, 60, cfg.window_mm), per_seed=False)
+    assert gpu["stats"]["n_pool"] <= gpu["stats"]["pool_cap"]
+    assert gpu["best_seed"][0] == 0 and gpu["best_n_match"][0] == 0 and gpu["best_chi2"][0] == 0.0
+    assert gpu["best_seed"][1] >= 0
+
+
 def test_single_seed_and_step_cap(setup):
     cfg, geom, field, events, grids, sc = setup
     ev = events[1]
