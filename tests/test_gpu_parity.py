@@ -106,6 +106,32 @@ def _hough_edge_votes(geom, ev, zref, hp, bins):
     return n
 
 
+@pytest.mark.parametrize("n_events", [1, 3, 6])
+def test_hough_accumulator_is_independent_of_the_batch_size(torch_cuda, n_events):
+    """The accumulator of an event does not depend on what else is in the batch (one grid row per event), and the
+    first and last event's equal the oracle's up to votes on the tolerance edge."""
+    cfg, geom, field, events, _ = U.make_workload(3, n_events=6)
+    events = events[:n_events]
+    sc = api.SeedScanner(geom, field)
+    off, w, d = synth.pack_hits(events)
+    E = sc.upload(off, w, d)
+    zref = [float(ev.seed[1]) for ev in events]
+    h = sc.hough(E, zref, want_accum=True)
+    one = api.SeedScanner(geom, field)
+    o1, w1, d1 = synth.pack_hits(events[:1])
+    h1 = one.hough(one.upload(o1, w1, d1), zref[:1], want_accum=True)
+    assert np.array_equal(h["accum"][0], h1["accum"][0]) and np.array_equal(h["peak"][0], h1["peak"][0])
+    bound = oracle.Bound(geom, field, U.oracle_params(cfg))
+    for e in (0, n_events - 1):
+        ho = oracle.hough(bound, events[e].wire_id, events[e].drift_mm, zref=float(np.float32(zref[e])))
+        diff = np.argwhere(h["accum"][e] != ho["accum"])
+        assert diff.shape[0] < 400
+        if diff.shape[0]:
+            assert _hough_edge_votes(geom, events[e], float(np.float32(zref[e])), B.HOUGH_DEFAULT,
+                                     [tuple(x) for x in diff]) >= diff.shape[0]
+    sc.close(); one.close()
+
+
 def test_cfg2_hough_ranges_eloss_full_size(torch_cuda):
     cfg, geom, field, events, _ = U.make_workload(2)
     ev = events[0]
