@@ -35,7 +35,7 @@ struct ScanArgs {
     double kq;                 // kappa * charge
     float kq_rel;              // kq / fl32(kq) - 1: the systematic part of a = fl32(kq) / p (energy-loss path)
     double h6_64;              // h / 6 in fp64 (for the systematic-rounding correction)
-    float lambda, inv_lambda, eloss_h;
+    float lambda, inv_lambda, eloss_h, window;
     float u2_lo, u2_hi;        // lookup band in u^2, widened by (K - 1) h
     float uz, inv_uz;          // cos(eps) of the canonical wire table (one |stereo| for all layers)
     float delta_max, b_max, hold_path;   // bounds behind g_dead (see consider())
@@ -67,23 +67,42 @@ __device__ __forceinline__ void slot_push(Slots &S, int w, float g)
 struct LookupCtx {         // the vertex a lookup is made from
     float x, xl, y, yl, z, Tx, Ty, Tz;     // the vertex itself: g of a new slot is evaluated here
     float cz, phi, g_dead, g_far;          // height and azimuth of the lookup centre
+    float curv;                            // |a| B_max (0: no pruning by distance, tight curls)
 };
 
 // a candidate with a hit becomes a live slot unless the track has already passed it for good: once g exceeds
 // g_dead it cannot return to <= 0 while the wire is in reach (g' >= |T_perp|^2 - |delta| |T'| >= -(|delta| |a| B)^2 / 4)
-__device__ __forceinline__ void consider(const ScanArgs &A, const uint32_t *s_bits, int w, const LookupCtx &V, Slots &S,
-                                         uint32_t &cnt)
+__device__ __forceinline__ void consider(const ScanArgs &A, const uint32_t *s_bits, const float *drift_e, int w,
+                                         const LookupCtx &V, Slots &S, uint32_t &cnt)
 {
     if (!((s_bits[w >> 5] >> (w & 31)) & 1u)) return;
     float ex, ey, eu;
     cnt += 1u;
-    const float g = wire_g(__ldg(A.gd.wire4 + w), A.uz, A.inv_uz, V.x, V.xl, V.y, V.yl, V.z, V.Tx, V.Ty, V.Tz, ex, ey, eu);
-    if (g <= V.g_dead && g > V.g_far) slot_push(S, w, g);
+    const float4 wr = __ldg(A.gd.wire4 + w);
+    const float g = wire_g(wr, A.uz, A.inv_uz, V.x, V.xl, V.y, V.yl, V.z, V.Tx, V.Ty, V.Tz, ex, ey, eu);
+    if (!(g <= V.g_dead && g > V.g_far)) return;
+    // A wire still ahead (g <= 0) is approached to D^2 = |delta|^2 - g^2 / |T_w|^2 along the tangent (T_w: T without its
+    // component along the wire), after a path s = -g / |T_w|^2 over which the track leaves its tangent by at most
+    // |a| B s^2 / 2.  Distance to a line is 1-Lipschitz, so the true closest approach differs from D by no more than
+    // that; if the drift circle cannot be met within the window even so, the wire is not made a live slot.
+    if (g <= 0.0f && V.curv > 0.0f) {
+        const float uT = fmaf(wr.z, V.Tx, fmaf(wr.w, V.Ty, A.uz * V.Tz));
+        const float tw2 = fmaf(-uT, uT, 1.0f);
+        if (tw2 > 0.25f) {
+            const float sp = __fdividef(g, tw2);                       // -s
+            const float D2 = fmaxf(fmaf(-g, sp, fmaf(ex, ex, fmaf(ey, ey, -eu * eu))), 0.0f);
+            const float tol = fmaf(0.6f * V.curv, sp * sp, A.window + 0.05f);
+            const float d = __ldg(drift_e + w);
+            const float hi = d + tol, lo = d - tol;
+            if (D2 > hi * hi || (lo > 0.0f && D2 < lo * lo)) return;
+        }
+    }
+    slot_push(S, w, g);
 }
 
 // cells kc and its nearer neighbour of layer j around azimuth phi at height z -> push those with a hit
-__device__ __forceinline__ void lookup_layer(const ScanArgs &A, const LayerDev *s_layer, const uint32_t *s_bits, int j,
-                                             const LookupCtx &V, Slots &S, uint32_t &cnt)
+__device__ __forceinline__ void lookup_layer(const ScanArgs &A, const LayerDev *s_layer, const uint32_t *s_bits,
+                                             const float *drift_e, int j, const LookupCtx &V, Slots &S, uint32_t &cnt)
 {
     if ((unsigned)j >= (unsigned)A.gd.n_layers) return;
     const LayerDev L = s_layer[j];
@@ -96,8 +115,8 @@ __device__ __forceinline__ void lookup_layer(const ScanArgs &A, const LayerDev *
     int k2 = k1 + ((kf - kn) >= 0.0f ? 1 : -1);
     k1 += (k1 < 0) ? L.n : 0; k1 += (k1 < 0) ? L.n : 0; k1 -= (k1 >= L.n) ? L.n : 0;
     k2 += (k2 < 0) ? L.n : 0; k2 += (k2 < 0) ? L.n : 0; k2 -= (k2 >= L.n) ? L.n : 0;
-    consider(A, s_bits, L.offset + k1, V, S, cnt);
-    consider(A, s_bits, L.offset + k2, V, S, cnt);
+    consider(A, s_bits, drift_e, L.offset + k1, V, S, cnt);
+    consider(A, s_bits, drift_e, L.offset + k2, V, S, cnt);
 }
 
 struct Vtx {               // position part of a step vertex (hi + the lo of x, y that the wire offset uses)
@@ -236,9 +255,10 @@ __global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
                     // nor can a wire own an approach before the next lookup if g is still far below zero: g grows by at
                     // most h (1 + |delta| |a| B) per step (g' = 1 - (T.u)^2 + delta . T')
                     V.g_far = -fmaf((float)kcount * h, 1.0f + cbend, 0.25f);
+                    V.curv = tight ? 0.0f : (ELOSS ? 1.05f : 1.0f) * fabsf(a) * A.b_max;
                 }
-                lookup_layer(A, s_layer, s_bits, jc, V, S, cnt);
-                lookup_layer(A, s_layer, s_bits, j2, V, S, cnt);
+                lookup_layer(A, s_layer, s_bits, drift_e, jc, V, S, cnt);
+                lookup_layer(A, s_layer, s_bits, drift_e, j2, V, S, cnt);
             }
         }
         kcount -= 1;
@@ -402,7 +422,7 @@ cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0
     A.h_6 = (float)(h / 6.0); A.h2_6 = (float)(h * h / 6.0);
     A.kq = CDC_KAPPA * (double)L.charge; A.h6_64 = h / 6.0;
     A.kq_rel = (float)(A.kq / (double)(float)A.kq - 1.0);
-    A.lambda = L.lambda; A.inv_lambda = 1.0f / L.lambda; A.eloss_h = L.eloss_h;
+    A.lambda = L.lambda; A.inv_lambda = 1.0f / L.lambda; A.eloss_h = L.eloss_h; A.window = sqrtf(L.lambda) * 1.0001f;
     A.u2_lo = L.u2_lo; A.u2_hi = L.u2_hi; A.uz = L.uz; A.inv_uz = L.inv_uz; A.lookup_every = L.lookup_every; A.lookahead = L.lookahead; A.lookup_every_tight = L.lookup_every_tight;
     A.delta_max = L.delta_max; A.b_max = L.b_max; A.hold_path = L.hold_path;
     A.max_steps = L.max_steps; A.margin = L.margin;
