@@ -156,7 +156,7 @@ __device__ __forceinline__ void slot_step(const ScanArgs &A, const float *drift_
 // defined through m_n), for the debug record, and when a held wire could be scored from a vertex inside R0; otherwise
 // every vertex a wire can be scored from lies in the gas (host check in launch_seed_scan) and they are dead weight.
 template <int FIELD, bool ELOSS, bool TRACK>
-__global__ void __launch_bounds__(kBlock) seed_scan_kernel(const ScanArgs A)
+__global__ void __launch_bounds__(kBlock, FIELD == 0 ? 8 : 0) seed_scan_kernel(const ScanArgs A)
 {
     __shared__ LayerDev s_layer[CDC_MAX_LAYERS];
     __shared__ uint32_t s_bits[kMaxBitWords];
