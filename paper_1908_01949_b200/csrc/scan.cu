@@ -215,7 +215,8 @@ __global__ void __launch_bounds__(kBlock, FIELD == 0 ? 8 : 0) seed_scan_kernel(c
         }
     }
     // p <= 1 MeV/c ends a track after its first step (C7)
-    const int max_steps = (p0h > 1.0f) ? A.max_steps : min(A.max_steps, 1);
+    // (a thread beyond the grid takes no step: its `valid` folded into the step cap keeps the loop test to one compare)
+    const int max_steps = !valid ? 0 : ((p0h > 1.0f) ? A.max_steps : min(A.max_steps, 1));
 
     uint32_t nm = 0, tests = 0, cnt = 0, lookups = 0;
     float chi2 = 0.0f;
@@ -226,7 +227,7 @@ __global__ void __launch_bounds__(kBlock, FIELD == 0 ? 8 : 0) seed_scan_kernel(c
     S.n = 0; S.w0 = S.w1 = S.w2 = S.w3 = 0; S.g0 = S.g1 = S.g2 = S.g3 = 0.0f;
 
 #pragma unroll 2
-    while (valid && n < max_steps) {
+    while (n < max_steps) {
         // ---- A5: every K steps, the wires near r_n that carry a hit -> slots, with g at this vertex
         if (kcount == 0) {
             // centre of the next K steps (straight-line prediction; the arc's sagitta is in the host's margin); a seed

@@ -47,6 +47,25 @@ def test_cfg0_full_grid_every_seed(torch_cuda):
     print(f"cfg0: {listed} listed threshold exceptions of {st['n_seeds']} seeds")
 
 
+@pytest.mark.parametrize("window,h,noise", [(3.0, 2.0, 0.30), (0.3, 4.0, 0.30), (5.0, 1.0, 0.15)])
+def test_wide_and_narrow_windows_dense_noise_every_seed(torch_cuda, window, h, noise):
+    """The lookup keeps a wire out of the live slots when a bound says it cannot own a matching approach before the
+    next lookup (too far ahead in g; drift circle out of reach).  The bounds depend on the window, the step and the
+    curvature: every seed of a two-turn event with dense noise is compared at a wide, a narrow and a very wide window."""
+    import dataclasses
+    cfg = dataclasses.replace(synth.CONFIGS[1], window_mm=window, h_mm=h, max_steps=int(3000 * 2.0 / h))
+    geom = synth.make_geometry(); field = synth.make_uniform_field()
+    ev = synth.generate_events(cfg, geom, field, 1, noise=noise)[0]
+    grid = synth.truth_anchored_grid(ev.seed, 7)[0]
+    sc = api.SeedScanner(geom, field)
+    gpu, off = _scan_all(sc, [ev], [grid], cfg)
+    orc = oracle.scan_parallel(geom, field, U.oracle_params(cfg), ev.wire_id, ev.drift_mm, grid)
+    listed = U.compare_scan(cfg, geom, field, ev, grid, gpu, orc, np.arange(grid.n_seeds))
+    U.check_best(cfg, geom, field, ev, grid, gpu, orc_full=orc)
+    assert int(orc["n_match"].max()) >= 20
+    print(f"window {window} mm, h {h} mm: {len(listed)} listed threshold exceptions of {grid.n_seeds} seeds")
+
+
 # ------------------------------------------------------------------ config 1: full size, sampled
 def test_cfg1_full_size_sampled(torch_cuda):
     cfg, geom, field, events, grids = U.make_workload(1)
