@@ -89,7 +89,7 @@ __device__ __forceinline__ void consider(const ScanArgs &A, const uint32_t *s_bi
         const float uT = fmaf(wr.z, V.Tx, fmaf(wr.w, V.Ty, A.uz * V.Tz));
         const float tw2 = fmaf(-uT, uT, 1.0f);
         if (tw2 > 0.25f) {
-            const float sp = __fdividef(g, tw2);                       // -s
+            const float sp = g * rcp_normal(tw2);                      // -s
             const float D2 = fmaxf(fmaf(-g, sp, fmaf(ex, ex, fmaf(ey, ey, -eu * eu))), 0.0f);
             const float tol = fmaf(0.6f * V.curv, sp * sp, A.window + 0.05f);
             const float d = __ldg(drift_e + w);
@@ -241,7 +241,7 @@ __global__ void __launch_bounds__(kBlock, FIELD == 0 ? 8 : 0) seed_scan_kernel(c
             const float u2 = fmaf(cx, cx, fmaf(cy, cy, -zeta * zeta));
             if (u2 > A.u2_lo && u2 < A.u2_hi) {
                 lookups += 1u;
-                const float u = u2 * rsqrtf(u2);
+                const float u = u2 * rsqrt_normal(u2);                  // u2 > u2_lo > 0
                 const float fj = (u - A.gd.r_first) * A.gd.inv_pitch;
                 const float jn = rintf(fj);
                 const int jc = (int)jn;

@@ -5,12 +5,27 @@
 
 namespace {
 
+// MUFU.RSQ / MUFU.RCP without the denormal-input scaling that rsqrtf() / __fdividef() wrap around them: only for
+// arguments known to be normal numbers (same result there)
+__device__ __forceinline__ float rsqrt_normal(float x)
+{
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float rcp_normal(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
 // atan2 good to ~2e-5 rad: it only selects candidate cells (a superset with ~7 mm of slack, reading C8).
 __device__ __forceinline__ float coarse_atan2(float y, float x)
 {
     float ax = fabsf(x), ay = fabsf(y);
     float mx = fmaxf(ax, ay), mn = fminf(ax, ay);
-    float t = __fdividef(mn, mx);
+    float t = mn * rcp_normal(fmaxf(mx, 1e-30f));
     float t2 = t * t;
     float p = fmaf(t2, -0.0117212f, 0.05265332f);
     p = fmaf(p, t2, -0.11643287f);
@@ -33,7 +48,7 @@ __device__ __forceinline__ void field_at(const FieldDev &F, float x, float y, fl
         // validated at create time: the table covers every point a live track or its stages can reach, so the
         // cell index needs no lower clamp; the unsigned min only keeps a non-finite state inside the allocation
         const float rho2 = fmaf(x, x, y * y);
-        const float inv_rho = rsqrtf(fmaxf(rho2, 1e-30f));
+        const float inv_rho = rsqrt_normal(fmaxf(rho2, 1e-30f));
         const float rho = rho2 * inv_rho;
         const float fr = fmaf(rho, F.inv_dr, F.cr), fz = fmaf(z, F.inv_dz, F.cz);
         const unsigned ir = min((unsigned)__float2int_rd(fr), (unsigned)(F.nr - 2));
