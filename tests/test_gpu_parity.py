@@ -66,6 +66,24 @@ def test_wide_and_narrow_windows_dense_noise_every_seed(torch_cuda, window, h, n
     print(f"window {window} mm, h {h} mm: {len(listed)} listed threshold exceptions of {grid.n_seeds} seeds")
 
 
+@pytest.mark.parametrize("cfg_id,n_events,grid_n,gen_kw", [(1, 4, 8, {}), (3, 4, 7, {}), (3, 3, 7, dict(noise=0.4, sigma_drift=0.5))])
+def test_other_events_every_seed(torch_cuda, cfg_id, n_events, grid_n, gen_kw):
+    """Every seed of further events (other generator seeds, denser noise, wider smearing), one batch per case."""
+    cfg = synth.CONFIGS[cfg_id]
+    geom = synth.make_geometry()
+    field = synth.make_uniform_field() if cfg.field_kind == 0 else synth.make_table_field()
+    events = synth.generate_events(cfg, geom, field, n_events, first_event=100, **gen_kw)
+    grids = [synth.truth_anchored_grid(ev.seed, grid_n)[0] for ev in events]
+    sc = api.SeedScanner(geom, field)
+    gpu, off = _scan_all(sc, events, grids, cfg)
+    o = 0
+    for e, (ev, grid) in enumerate(zip(events, grids)):
+        orc = oracle.scan_parallel(geom, field, U.oracle_params(cfg), ev.wire_id, ev.drift_mm, grid)
+        U.compare_scan(cfg, geom, field, ev, grid, gpu, orc, np.arange(grid.n_seeds), offset=o)
+        U.check_best(cfg, geom, field, ev, grid, gpu, e=e, hit_slice=slice(off[e], off[e + 1]), orc_full=orc)
+        o += grid.n_seeds
+
+
 # ------------------------------------------------------------------ config 1: full size, sampled
 def test_cfg1_full_size_sampled(torch_cuda):
     cfg, geom, field, events, grids = U.make_workload(1)
