@@ -83,5 +83,16 @@ class SeedScanner:
         return B.cdc_find_tracks_host(self.geometry, hit_offsets, wire_id, drift_mm, B.grid_specs(grids), params,
                                       hp, zref)
 
+    def refine(self, events: B.Events, grids: Sequence, params: B.ScanParams, n_parents: int = 8,
+               n_iterations: int = 10, **kw) -> dict:
+        """Coarse-to-fine refinement around the best seeds of `grids` (cdc_refine_tracks)."""
+        return B.cdc_refine_tracks(self.geometry, events, B.grid_specs(grids), params, n_parents=n_parents,
+                                   n_iterations=n_iterations, **kw)
+
+    def peel(self, events: B.Events, grids0: Sequence, params: B.ScanParams, n: Sequence[int],
+             half_width: Sequence[float], **kw) -> dict:
+        """Turn-partition peeling from partition 0's grids (cdc_peel_turns)."""
+        return B.cdc_peel_turns(self.geometry, events, B.grid_specs(grids0), params, n, half_width, **kw)
+
     def close(self):
         self.geometry.close()
