@@ -118,6 +118,14 @@ def rkn_step(bound: Bound, a: float, h: float, r, T):
     return rn, Tn
 
 
+def rkn_step_err(bound: Bound, a: float, h: float, r, T):
+    """One RKN step and the local error estimate h^2 max|k1 - k2 - k3 + k4| of PAPER.md ref. [5] (reading C19)."""
+    r = np.ascontiguousarray(r, dtype=np.float64); T = np.ascontiguousarray(T, dtype=np.float64)
+    rn = np.zeros(3); Tn = np.zeros(3); err = C.c_double()
+    lib().orc_rkn_step_err(C.byref(bound.f), C.c_double(a), C.c_double(h), _p(r), _p(T), _p(rn), _p(Tn), C.byref(err))
+    return rn, Tn, float(err.value)
+
+
 def eval_seed(bound: Bound, wire_id, drift, seed, mode: int = 1, records: bool = False,
               rec_slack: float = 0.0, trajectory: bool = False):
     """Evaluate one seed.  Returns dict(n_match, chi2, n_steps, turns, m_gas, r, T, p[, rec][, traj])."""

@@ -146,6 +146,36 @@ void orc_rkn_step(const orc_field *f, double a, double h, const double *r, const
     }
 }
 
+/* The same step, plus the local error estimate of the adaptive Runge-Kutta-Nystroem propagator of PAPER.md ref. [5]
+ * (Lund et al., JINST 4 P04001): err = h^2 max_i |k1_i - k2_i - k3_i + k4_i|, each component
+ * evaluated left to right (reading C19).  rn, Tn are bit-equal to orc_rkn_step's. */
+void orc_rkn_step_err(const orc_field *f, double a, double h, const double *r, const double *T,
+                      double *rn, double *Tn, double *err)
+{
+    double B[3], k1[3], k2[3], k3[3], k4[3], q[3], U[3];
+    double emax = 0.0;
+    int i;
+    orc_field_at(f, r[0], r[1], r[2], B);
+    cross_scaled(a, T, B, k1);
+    for (i = 0; i < 3; ++i) q[i] = r[i] + (h / 2.0) * T[i] + (h * h / 8.0) * k1[i];
+    orc_field_at(f, q[0], q[1], q[2], B);
+    for (i = 0; i < 3; ++i) U[i] = T[i] + (h / 2.0) * k1[i];
+    cross_scaled(a, U, B, k2);
+    for (i = 0; i < 3; ++i) U[i] = T[i] + (h / 2.0) * k2[i];
+    cross_scaled(a, U, B, k3);
+    for (i = 0; i < 3; ++i) q[i] = r[i] + h * T[i] + (h * h / 2.0) * k3[i];
+    orc_field_at(f, q[0], q[1], q[2], B);
+    for (i = 0; i < 3; ++i) U[i] = T[i] + h * k3[i];
+    cross_scaled(a, U, B, k4);
+    for (i = 0; i < 3; ++i) {
+        double e = k1[i] - k2[i] - k3[i] + k4[i];
+        rn[i] = r[i] + h * T[i] + (h * h / 6.0) * (k1[i] + k2[i] + k3[i]);
+        Tn[i] = T[i] + (h / 6.0) * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
+        if (fabs(e) > emax) emax = fabs(e);
+    }
+    *err = h * h * emax;
+}
+
 /* ---- C9: offset of a point from a wire line, and g = delta . T ---------- */
 static void wire_delta(const float *w, const double *r, double *delta, double *tpar)
 {

@@ -28,6 +28,17 @@ The crossing point of step 6, between the vertices r_n (rho < R0) and r_{n+1} (r
     A = dx dx + dy dy,  B = x dx + y dy,  C = x x + y y - R0 R0,  tau = (-B + sqrt(B B - A C)) / A,
     position r_n + tau d,  direction U / |U| with U = T_n + tau (T_{n+1} - T_n),  momentum p_n (no loss below R0),
 every expression evaluated left to right in fp64; theta = atan2(y, x) of the position (libm).
+
+Adaptive extrapolation (extrap_tol > 0; reading C19): PAPER.md:55 takes its propagator from ref. [5] (Lund et al.,
+PAPER.md:151), whose Runge-Kutta-Nystroem step carries the local error estimate err = h^2 max_i |k1_i - k2_i - k3_i +
+k4_i|.  Between two partitions nothing is scored, so step 6 may take longer steps where that estimate allows it:
+    the step length starts at h and is always h 2^j, h <= h 2^j <= h_max;
+    a trial step with err > tol is repeated with half the length (never below h);
+    a trial step that crosses rho = R0 outward with a length above h is repeated with half the length (the crossing
+    point is always taken on a chord of length h, as in the fixed-step form);
+    after an accepted step with err <= tol / 32 the length doubles if that stays <= h_max (err grows ~16-fold);
+    momentum: p = p0 - eloss * (path of the accepted steps that started at rho >= R0), the sum being exact in fp64.
+Only accepted steps count against max_steps.  extrap_tol = 0 is the fixed-step form above.
 Plain Python loops around the C oracle's single RKN step, exhaustive scan, arg max and labels.
 """
 from __future__ import annotations
@@ -37,7 +48,7 @@ import types
 
 import numpy as np
 
-from . import Bound, argmax, labels, rkn_step, scan_parallel, seed_of_index
+from . import Bound, argmax, labels, rkn_step, rkn_step_err, scan_parallel, seed_of_index
 
 KAPPA = 0.299792458          # reading C1 (same constant as cdc_oracle.c)
 
@@ -45,8 +56,66 @@ STATUS = {1: "fewer than min_hits unclassified hits", 2: "partition with fewer t
           3: "max_partitions reached", 4: "track ended before the next entrance"}
 
 
-def next_entrance(geom, field, params: dict, seed, max_steps: int):
+def _crossing(r, T, rn, Tn, p, R0):
+    d = [rn[i] - r[i] for i in range(3)]
+    A = d[0] * d[0] + d[1] * d[1]
+    B = r[0] * d[0] + r[1] * d[1]
+    Cc = r[0] * r[0] + r[1] * r[1] - R0 * R0
+    tau = (-B + math.sqrt(B * B - A * Cc)) / A
+    pos = [r[i] + tau * d[i] for i in range(3)]
+    U = [T[i] + tau * (Tn[i] - T[i]) for i in range(3)]
+    nU = math.sqrt(U[0] * U[0] + U[1] * U[1] + U[2] * U[2])
+    return pos + [p * (U[i] / nU) for i in range(3)]
+
+
+def next_entrance_adaptive(geom, field, params: dict, seed, max_steps: int, tol: float, h_max: float, trace=None):
+    """Step 6 with the step-doubling controller on the error estimate of ref. [5] (module docstring).
+    trace (optional list): receives the length of every accepted step."""
+    bound = Bound(geom, field, params)
+    h0 = float(params["h"]); eloss = float(params.get("eloss", 0.0))
+    kq = KAPPA * float(int(params.get("charge", -1)))
+    R0 = float(geom.R0_mm); z_half = float(geom.z_half_mm); r_out = float(geom.r_out_mm)
+    th, z0, px, py, pz = (float(v) for v in seed)
+    r = [R0 * math.cos(th), R0 * math.sin(th), z0]                                   # C4
+    p0 = math.sqrt(px * px + py * py + pz * pz)
+    T = [px / p0, py / p0, pz / p0]
+    p = p0
+    n = 0; s_gas = 0.0; hc = h0
+    c_n = True
+    while n < max_steps:
+        a = kq / p
+        rn, Tn, err = rkn_step_err(bound, a, hc, r, T)
+        rn = [float(v) for v in rn]; Tn = [float(v) for v in Tn]
+        if err > tol and hc > h0:
+            hc = hc / 2.0
+            continue
+        c_next = rn[0] * rn[0] + rn[1] * rn[1] >= R0 * R0
+        if (not c_n) and c_next and hc > h0:
+            hc = hc / 2.0
+            continue
+        s_next = s_gas + hc if c_n else s_gas                                        # C6
+        p_next = p0 - eloss * s_next
+        if (not c_n) and c_next:                                                     # C7: a new turn starts here
+            return _crossing(r, T, rn, Tn, p_next, R0)
+        if trace is not None:
+            trace.append(hc)
+        r, T = rn, Tn
+        n += 1
+        p = p_next; s_gas = s_next
+        c_n = c_next
+        if abs(r[2]) > z_half: break
+        if r[0] * r[0] + r[1] * r[1] > r_out * r_out: break
+        if not (p > 1.0): break
+        if not all(math.isfinite(v) for v in r + T): break
+        if err <= tol / 32.0 and hc * 2.0 <= h_max:
+            hc = hc * 2.0
+    return None
+
+
+def next_entrance(geom, field, params: dict, seed, max_steps: int, tol: float = 0.0, h_max: float = 0.0):
     """Step 6.  Returns (x, y, z, px, py, pz) at the next outward crossing of rho = R0, or None."""
+    if tol > 0.0:
+        return next_entrance_adaptive(geom, field, params, seed, max_steps, tol, h_max)
     bound = Bound(geom, field, params)
     h = float(params["h"]); eloss_h = float(params.get("eloss", 0.0)) * h
     kq = KAPPA * float(int(params.get("charge", -1)))
@@ -67,15 +136,7 @@ def next_entrance(geom, field, params: dict, seed, max_steps: int):
         p_next = p0 - eloss_h * float(m)
         c_next = rn[0] * rn[0] + rn[1] * rn[1] >= R0 * R0
         if (not c_n) and c_next:                                                     # C7: a new turn starts here
-            d = [rn[i] - r[i] for i in range(3)]
-            A = d[0] * d[0] + d[1] * d[1]
-            B = r[0] * d[0] + r[1] * d[1]
-            Cc = r[0] * r[0] + r[1] * r[1] - R0 * R0
-            tau = (-B + math.sqrt(B * B - A * Cc)) / A
-            pos = [r[i] + tau * d[i] for i in range(3)]
-            U = [T[i] + tau * (Tn[i] - T[i]) for i in range(3)]
-            nU = math.sqrt(U[0] * U[0] + U[1] * U[1] + U[2] * U[2])
-            return pos + [p_next * (U[i] / nU) for i in range(3)]
+            return _crossing(r, T, rn, Tn, p_next, R0)
         r, T = rn, Tn
         n += 1
         p = p_next
@@ -101,7 +162,8 @@ def centred_grid(centre, half_width, n):
 
 
 def peel(geom, field, params: dict, wire_id, drift, grid0, n, half_width, max_partitions: int = 4,
-         min_hits: int = 10, min_classified: int = 5, extrap_max_steps: int = 3000, n_proc=None):
+         min_hits: int = 10, min_classified: int = 5, extrap_max_steps: int = 3000, extrap_tol: float = 0.0,
+         extrap_h_max: float = 0.0, n_proc=None):
     """Returns dict(partition (H,) int32: index of the partition a hit was classified into or -1, seeds (P, 5),
     n_match (P,), chi2 (P,), S (P,), status, centres: the extrapolated grid centres (P - 1 or P, 5))."""
     wire_id = np.asarray(wire_id, dtype=np.int32); drift = np.asarray(drift, dtype=np.float32)
@@ -131,7 +193,7 @@ def peel(geom, field, params: dict, wire_id, drift, grid0, n, half_width, max_pa
             status = 1; break
         if k + 1 == max_partitions:
             status = 3; break
-        nx = next_entrance(geom, field, params, seed, extrap_max_steps)
+        nx = next_entrance(geom, field, params, seed, extrap_max_steps, extrap_tol, extrap_h_max)
         if nx is None:
             status = 4; break
         centre = [math.atan2(nx[1], nx[0]), nx[2], nx[3], nx[4], nx[5]]

@@ -69,6 +69,59 @@ def test_next_entrance_lies_on_the_chord_of_the_c_oracles_trajectory_and_loses_t
     assert np.dot(u, traj[n, 3:]) > 1 - 1e-4 and np.dot(u, traj[n + 1, 3:]) > 1 - 1e-4
 
 
+def test_error_estimate_of_the_adaptive_step_equals_its_uniform_field_closed_form():
+    # reading C19 / PAPER.md ref. [5]: err = h^2 max_i |k1 - k2 - k3 + k4|_i.  In a uniform field k = c J U with
+    # c = a B_z and J (Ux, Uy) = (Uy, -Ux); expanding the four stages gives
+    #   k1 - k2 - k3 + k4 = -(c^3 h^2 / 4) J T + (c^4 h^3 / 4) T_xy        (z component 0)
+    # and the step itself must be the plain step bit for bit
+    geom = synth.make_geometry(); field = synth.make_uniform_field(0.9)
+    bound = oracle.Bound(geom, field, dict(h=2.0, max_steps=10, window=1.0))
+    rng = np.random.default_rng(5)
+    for _ in range(20):
+        T = rng.normal(size=3); T /= np.linalg.norm(T)
+        r = rng.uniform(-600, 600, size=3)
+        a = -0.299792458 / rng.uniform(20.0, 110.0); h = float(rng.choice([1.0, 2.0, 4.0, 16.0]))
+        rn, Tn, err = oracle.rkn_step_err(bound, a, h, r, T)
+        rn0, Tn0 = oracle.rkn_step(bound, a, h, r, T)
+        assert np.array_equal(rn, rn0) and np.array_equal(Tn, Tn0)
+        c = a * 0.9
+        e = -(c ** 3 * h ** 2 / 4.0) * np.array([T[1], -T[0]]) + (c ** 4 * h ** 3 / 4.0) * T[:2]
+        assert abs(err - h * h * np.abs(e).max()) <= 1e-6 * err + 1e-22
+
+
+def test_adaptive_extrapolation_takes_fewer_longer_steps_to_the_same_entrance():
+    cfg, geom, field, ev = _two_turn_event()
+    params = dict(h=cfg.h_mm, max_steps=cfg.max_steps, window=cfg.window_mm)
+    fixed = np.array(OP.next_entrance(geom, field, params, ev.seed, 3000))
+    tr = []
+    tiny = np.array(OP.next_entrance_adaptive(geom, field, params, ev.seed, 3000, 1e-12, 32.0, trace=tr))
+    assert set(tr) == {cfg.h_mm} and np.array_equal(tiny, fixed)        # never below h: the fixed-step form itself
+    tr = []
+    ad = np.array(OP.next_entrance_adaptive(geom, field, params, ev.seed, 3000, 1e-3, 32.0, trace=tr))
+    assert set(tr) <= {2.0, 4.0, 8.0, 16.0, 32.0} and max(tr) >= 8.0 and len(tr) < 300
+    assert np.abs(ad[:3] - fixed[:3]).max() < 1e-4 and np.abs(ad[3:] - fixed[3:]).max() < 1e-5
+    assert abs(math.hypot(ad[0], ad[1]) - geom.R0_mm) < 1e-9
+    capped = []
+    OP.next_entrance_adaptive(geom, field, params, ev.seed, 3000, 1.0, 4.0, trace=capped)
+    assert max(capped) == 4.0                                            # h_max
+    # tabulated field: the estimate follows the field's variation, same entrance
+    cfg2 = synth.CONFIGS[2]
+    tf = synth.make_table_field()
+    ev2 = synth.generate_events(cfg2, geom, tf, 1)[0]
+    p2 = dict(h=cfg2.h_mm, max_steps=cfg2.max_steps, window=cfg2.window_mm)
+    f2 = np.array(OP.next_entrance(geom, tf, p2, ev2.seed, 3000))
+    a2 = np.array(OP.next_entrance(geom, tf, p2, ev2.seed, 3000, 1e-4, 16.0))
+    assert np.abs(a2[:3] - f2[:3]).max() < 1e-3 and np.abs(a2[3:] - f2[3:]).max() < 1e-4
+    # with energy loss the momentum is constant over a step (C6), so the step length enters at first order:
+    # the loss over one 16 mm step is 3.2e-3 MeV/c, 3e-5 of p, which bends ~1 m of path by ~0.02 mm; |p| itself
+    # differs by less than one step's loss
+    p2["eloss"] = cfg2.eloss_MeV_per_mm
+    f2 = np.array(OP.next_entrance(geom, tf, p2, ev2.seed, 3000))
+    a2 = np.array(OP.next_entrance(geom, tf, p2, ev2.seed, 3000, 1e-4, 16.0))
+    assert np.abs(a2[:3] - f2[:3]).max() < 0.05
+    assert abs(np.linalg.norm(a2[3:]) - np.linalg.norm(f2[3:])) <= 16.0 * cfg2.eloss_MeV_per_mm
+
+
 def test_centred_grid_nodes():
     g = OP.centred_grid([1.0, 2.0, 3.0, 4.0, 5.0], [0.5, 1.0, 0.0, 2.0, 4.0], [3, 5, 1, 2, 9])
     nodes = [[g.lo[a] + i * g.step[a] for i in range(int(g.n[a]))] for a in range(5)]
