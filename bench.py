@@ -402,7 +402,7 @@ def run_peel(args):
     steps = 1500
     P = B.scan_params(cfg.h_mm, steps, cfg.window_mm, cfg.eloss_MeV_per_mm)
     hw = [0.01, 26.0, 2.5, 2.5, 1.7]
-    ms = []
+    ms, ms_ad = [], []
     n0 = B.cdc_kernel_launch_count()
     for it in range(args.warmup + args.steps):
         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
@@ -413,7 +413,16 @@ def run_peel(args):
             n0 = B.cdc_kernel_launch_count()
         if it >= args.warmup:
             ms.append(e0.elapsed_time(e1))
-    launches = (B.cdc_kernel_launch_count() - n0) // max(args.steps, 1)
+    n1 = B.cdc_kernel_launch_count()
+    for it in range(args.warmup + args.steps):       # the same with the adaptive extrapolation between partitions
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); e0.record()
+        out_ad = B.cdc_peel_turns(sc.geometry, ev, B.grid_specs(grids), P, [8] * 5, hw, max_partitions=4,
+                                  extrap_tol=1e-4, extrap_h_max=16.0)
+        e1.record(); e1.synchronize()
+        if it >= args.warmup:
+            ms_ad.append(e0.elapsed_time(e1))
+    launches = (n1 - n0) // max(args.steps, 1)
     # Eq. (2), (3) against the generator's truth turns, by the library's own kernel (not part of the timed region)
     truth = torch.tensor(np.concatenate([e.truth_turn for e in events]).astype(np.int32), device="cuda")
     q = B.cdc_classification_quality(ev, 3, out["d_partition"], truth)
@@ -426,6 +435,8 @@ def run_peel(args):
     print(json.dumps({"measurement": "turn_peeling", "workload": args.workload, "events": len(events),
                       "seeds_partition0": int(grids[0].n_seeds), "seeds_next": 8 ** 5, "max_steps": steps,
                       "ms_per_call": t * 1e3, "events_per_s": len(events) / t, "kernel_launches_per_call": int(launches),
+                      "ms_per_call_adaptive_extrapolation": float(np.mean(ms_ad)),
+                      "adaptive_same_partitions": bool(np.array_equal(out["partition"], out_ad["partition"])),
                       "partitions_found": [int(v) for v in out["n_partitions"]], "true_turns": [e.n_turns for e in events],
                       "status": [int(v) for v in out["status"]], "events_with_all_turns": found,
                       "mean_efficiency": float(np.mean(eff)) if eff else None,

@@ -242,6 +242,11 @@ typedef struct {
     int32_t n[5];             /* nodes per axis of the grids of partitions 1.. (1..4096 each) */
     int32_t pad_;
     double half_width[5];
+    double extrap_tol_mm;     /* 0: the extrapolation uses the scan's fixed step h.  > 0: adaptive step (reading C19): */
+    double extrap_h_max_mm;   /*    step lengths h 2^j in [h, extrap_h_max_mm], controlled by the local error estimate
+                               *    h^2 max|k1 - k2 - k3 + k4| of the paper's propagator reference [5]:
+                               *    halved on err > tol, doubled after err <= tol / 32; the crossing of rho = R0 is always
+                               *    taken on a chord of length h */
 } cdc_peel_params;
 int32_t cdc_peel_turns(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec *h_grids0,
                        const cdc_scan_params *params, const cdc_peel_params *pp, int32_t *h_n_partitions,

@@ -59,7 +59,8 @@ class RefineParams(C.Structure):
 
 class PeelParams(C.Structure):
     _fields_ = [("max_partitions", C.c_int32), ("min_hits", C.c_int32), ("min_classified", C.c_int32),
-                ("extrap_max_steps", C.c_int32), ("n", C.c_int32 * 5), ("pad_", C.c_int32), ("half_width", C.c_double * 5)]
+                ("extrap_max_steps", C.c_int32), ("n", C.c_int32 * 5), ("pad_", C.c_int32), ("half_width", C.c_double * 5),
+                ("extrap_tol_mm", C.c_double), ("extrap_h_max_mm", C.c_double)]
 
 
 class ScanStats(C.Structure):
@@ -277,12 +278,12 @@ def cdc_refine_tracks(geometry: Geometry, events: Events, grids: C.Array, params
 
 def cdc_peel_turns(geometry: Geometry, events: Events, grids0: C.Array, params: ScanParams, n: Sequence[int],
                    half_width: Sequence[float], max_partitions: int = 4, min_hits: int = 10, min_classified: int = 5,
-                   extrap_max_steps: int = 3000, stream=None) -> dict:
+                   extrap_max_steps: int = 3000, extrap_tol: float = 0.0, extrap_h_max: float = 0.0, stream=None) -> dict:
     """Turn-partition peeling.  Host (numpy) outputs; `partition` is read back from the device."""
     import torch
     E, P = events.n_events, int(max_partitions)
     pp = PeelParams(P, int(min_hits), int(min_classified), int(extrap_max_steps), (C.c_int32 * 5)(*[int(v) for v in n]), 0,
-                    (C.c_double * 5)(*[float(v) for v in half_width]))
+                    (C.c_double * 5)(*[float(v) for v in half_width]), float(extrap_tol), float(extrap_h_max))
     n_part = np.zeros(E, dtype=np.int32); status = np.zeros(E, dtype=np.int32)
     seeds = np.zeros((E, P, 5)); nm = np.zeros((E, P), dtype=np.uint32); chi2 = np.zeros((E, P)); centres = np.zeros((E, P, 5))
     d_part = torch.empty(max(events.n_hits, 1), dtype=torch.int32, device="cuda")

@@ -59,6 +59,10 @@ extern "C" int32_t cdc_peel_turns(const cdc_geometry *g, cdc_events *ev, const c
         if (!(pp->half_width[a] >= 0.0) || !isfinite(pp->half_width[a]))
             CDC_FAIL(CDC_ERR_INVALID, "cdc_peel_turns: half_width must be finite and >= 0");
     }
+    if (!(pp->extrap_tol_mm >= 0.0) || !isfinite(pp->extrap_tol_mm))
+        CDC_FAIL(CDC_ERR_INVALID, "cdc_peel_turns: extrap_tol_mm must be finite and >= 0");
+    if (pp->extrap_tol_mm > 0.0 && (!(pp->extrap_h_max_mm >= p->h_mm) || !isfinite(pp->extrap_h_max_mm)))
+        CDC_FAIL(CDC_ERR_INVALID, "cdc_peel_turns: adaptive extrapolation needs h <= extrap_h_max_mm < inf");
     if (ev->total_hits > 0 && !d_partition) CDC_FAIL(CDC_ERR_INVALID, "cdc_peel_turns: null d_partition");
     cudaStream_t s = (cudaStream_t)stream;
     Dev D(s);
@@ -97,6 +101,7 @@ extern "C" int32_t cdc_peel_turns(const cdc_geometry *g, cdc_events *ev, const c
     L.g = g->g64; L.n_events = E; L.W = ev->W; L.n_bit_words = ev->n_bit_words; L.max_hits_per_event = ev->max_hits_per_event;
     L.d_offsets = ev->d_offsets; L.d_wire_id = ev->d_wire_id; L.d_bits = ev->d_bits;
     L.h = p->h_mm; L.eloss = p->eloss_MeV_per_mm; L.kq = CDC_KAPPA * (double)p->charge; L.extrap_max_steps = pp->extrap_max_steps;
+    L.extrap_tol = pp->extrap_tol_mm; L.extrap_h_max = pp->extrap_h_max_mm;
     L.d_labels = d_labels; L.d_best_seed = d_best; L.d_active = d_active; L.d_partition = d_partition;
     L.d_counts = d_counts; L.d_next = d_next; L.d_next_ok = d_ok;
 

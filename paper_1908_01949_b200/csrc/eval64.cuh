@@ -99,6 +99,37 @@ __device__ __forceinline__ void rkn_step64(const Geom64 &g, double a, double h, 
     }
 }
 
+// The same step plus the local error estimate of the adaptive propagator of PAPER.md ref. [5] (reading C19):
+// err = h^2 max_i |k1_i - k2_i - k3_i + k4_i|, each component left to right.  General form only (rn, Tn as above).
+__device__ __forceinline__ void rkn_step64_err(const Geom64 &g, double a, double h, const double *r, const double *T,
+                                               double *rn, double *Tn, double *err)
+{
+    const double hh = h / 2.0, h28 = h * h / 8.0, h22 = h * h / 2.0, h26 = h * h / 6.0, h6 = h / 6.0;
+    double B[3], k1[3], k2[3], k3[3], k4[3], q[3], U[3];
+    field64(g, r[0], r[1], r[2], B);
+    lorentz64(a, T, B, k1);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { q[i] = r[i] + hh * T[i] + h28 * k1[i]; U[i] = T[i] + hh * k1[i]; }
+    field64(g, q[0], q[1], q[2], B);
+    lorentz64(a, U, B, k2);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) U[i] = T[i] + hh * k2[i];
+    lorentz64(a, U, B, k3);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { q[i] = r[i] + h * T[i] + h22 * k3[i]; U[i] = T[i] + h * k3[i]; }
+    field64(g, q[0], q[1], q[2], B);
+    lorentz64(a, U, B, k4);
+    double emax = 0.0;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const double e = k1[i] - k2[i] - k3[i] + k4[i];
+        rn[i] = r[i] + h * T[i] + h26 * (k1[i] + k2[i] + k3[i]);
+        Tn[i] = T[i] + h6 * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
+        if (fabs(e) > emax) emax = fabs(e);
+    }
+    *err = h * h * emax;
+}
+
 // reading C9: delta = d - (d.u) u with d = r - w0;  returns g = delta . T when T != nullptr
 __device__ __forceinline__ void wire_offset64(const float *w, const double *r, double *delta, double *tpar)
 {

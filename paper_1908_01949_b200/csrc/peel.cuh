@@ -12,6 +12,7 @@ struct PeelLaunch {
     int32_t axis_stride;
     double h, eloss, kq;
     int32_t extrap_max_steps;
+    double extrap_tol, extrap_h_max;  // tol > 0: adaptive extrapolation (reading C19)
     const int32_t *d_labels;          // hit -> turn labels of the partition's best seed
     const int64_t *d_best_seed;       // its linear index per event (-1: none)
     const int32_t *d_active;          // [E] 1 = the event is still being peeled

@@ -170,7 +170,7 @@ def test_peeling_stops_for_each_listed_reason():
     assert r["partition"].max() < r["seeds"].shape[0]
 
 
-def _gpu_vs_oracle(cfg_id, n_events, n0, n, max_steps, P=3, **gen_kw):
+def _gpu_vs_oracle(cfg_id, n_events, n0, n, max_steps, P=3, extrap_tol=0.0, extrap_h_max=0.0, **gen_kw):
     from paper_1908_01949_b200 import api, binding as B
     cfg = synth.CONFIGS[cfg_id]
     geom = synth.make_geometry()
@@ -184,12 +184,12 @@ def _gpu_vs_oracle(cfg_id, n_events, n0, n, max_steps, P=3, **gen_kw):
     params = dict(h=cfg.h_mm, max_steps=max_steps, window=cfg.window_mm, eloss=cfg.eloss_MeV_per_mm)
     Pg = B.scan_params(cfg.h_mm, max_steps, cfg.window_mm, cfg.eloss_MeV_per_mm)
     out = B.cdc_peel_turns(sc.geometry, E, B.grid_specs(grids), Pg, n, HALF_WIDTH, max_partitions=P, min_hits=10,
-                           min_classified=5, extrap_max_steps=3000)
+                           min_classified=5, extrap_max_steps=3000, extrap_tol=extrap_tol, extrap_h_max=extrap_h_max)
     assert np.array_equal(E.tables()[1], bits_before)                       # the events are handed back unchanged
     res = []
     for e, (ev, g0) in enumerate(zip(events, grids)):
         r = OP.peel(geom, field, params, ev.wire_id, ev.drift_mm, g0, n, HALF_WIDTH, max_partitions=P, min_hits=10,
-                    min_classified=5, extrap_max_steps=3000)
+                    min_classified=5, extrap_max_steps=3000, extrap_tol=extrap_tol, extrap_h_max=extrap_h_max)
         k = r["seeds"].shape[0]
         assert out["status"][e] == r["status"] and out["n_partitions"][e] == k, (e, out["status"][e], r["status"])
         assert np.array_equal(out["partition"][off[e]:off[e + 1]], r["partition"]), e       # bit-exact labels
@@ -224,6 +224,15 @@ def test_gpu_peeling_equals_oracle_table_field_mixed_turn_counts():
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("cfg_id,n_events,P", [(1, 2, 3), (2, 1, 4), (3, 4, 3)])
+def test_gpu_peeling_with_adaptive_extrapolation_equals_oracle(cfg_id, n_events, P):
+    # reading C19: step lengths up to 16 mm between the partitions; every step-size decision is taken in fp64 on both
+    # sides, so the extrapolated centres (hence everything after them) are still bit-equal
+    res = _gpu_vs_oracle(cfg_id, n_events, 6, [5, 5, 5, 5, 5], 1500, P=P, extrap_tol=1e-4, extrap_h_max=16.0)
+    assert any(r["centres"].shape[0] >= 1 for _, r in res)
+
+
+@pytest.mark.gpu
 def test_gpu_peeling_rejects_bad_arguments():
     from paper_1908_01949_b200 import api, binding as B
     cfg, geom, field, ev = _two_turn_event()
@@ -232,7 +241,8 @@ def test_gpu_peeling_rejects_bad_arguments():
     E = sc.upload(off, w, d)
     g = B.grid_specs([synth.truth_anchored_grid(ev.seed, 2)[0]])
     Pg = B.scan_params(cfg.h_mm, 500, cfg.window_mm)
-    for kw in (dict(max_partitions=0), dict(max_partitions=9), dict(min_hits=-1), dict(extrap_max_steps=0)):
+    for kw in (dict(max_partitions=0), dict(max_partitions=9), dict(min_hits=-1), dict(extrap_max_steps=0),
+               dict(extrap_tol=-1.0), dict(extrap_tol=1e-4, extrap_h_max=1.0), dict(extrap_tol=float("nan"))):
         with pytest.raises(B.CdcError):
             B.cdc_peel_turns(sc.geometry, E, g, Pg, [2] * 5, HALF_WIDTH, **kw)
     with pytest.raises(B.CdcError):
