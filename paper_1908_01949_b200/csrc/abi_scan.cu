@@ -198,6 +198,13 @@ extern "C" int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cd
         // |a| B_max < 1 / 20 mm per seed); tighter curls look up around r_n itself, every K0 steps
         const int K0 = std::max(1, std::min(1 + (int)floor((g->excl - reach) / p->h_mm), 16));
         L.lookup_every_tight = K0;
+        // vertex n + i lies i h along the arc: (i h - ahead) along the tangent from c and at most kappa (i h)^2 / 2 off
+        // it, so it stays within ahead + sag of c for every i <= K iff kappa <= 2 sqrt(sag^2 + 2 sag ahead) / (K h)^2
+        // (kappa = |a| B_max, the track's curvature bound); never above the old fixed 1 / 20 mm
+        {
+            const double Kh = K * p->h_mm;
+            L.tight_curv = (float)(ahead > 0.0 ? std::min(0.05, 0.98 * 2.0 * sqrt(sag * sag + 2.0 * sag * ahead) / (Kh * Kh)) : 0.05);
+        }
         const double grow = reach + 0.2 + std::max(ahead + sag, (K0 - 1) * p->h_mm);
         const double ulo = std::max(g->r[0] - grow, 0.0), uhi = g->r[g->n_layers - 1] + grow;
         L.u2_lo = (float)(ulo * ulo); L.u2_hi = (float)(uhi * uhi);

@@ -181,7 +181,8 @@ struct ScanLaunch {
     float u2_lo, u2_hi, uz, inv_uz;  // lookup band (widened for the lookup cadence), cos(eps)
     int32_t lookup_every;            // K: steps per layer/cell lookup
     float lookahead;                 // the lookup is centred on r_n + lookahead * T_n (the middle of the next K steps)
-    int32_t lookup_every_tight;      // K for tightly curling seeds (radius < 20 mm): lookup centred on r_n itself
+    int32_t lookup_every_tight;      // K for tightly curling seeds: lookup centred on r_n itself
+    float tight_curv;                // |a| B_max at and above which a seed counts as tightly curling (host: sagitta margin)
     float delta_max, b_max, hold_path;   // largest |delta| of a held wire, largest |B|, longest path a wire stays held
 };
 cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0, cudaEvent_t k1);

@@ -40,7 +40,7 @@ struct ScanArgs {
     float uz, inv_uz;          // cos(eps) of the canonical wire table (one |stereo| for all layers)
     float delta_max, b_max, hold_path;   // bounds behind g_dead (see consider())
     int32_t max_steps, lookup_every, lookup_every_tight;
-    float lookahead;
+    float lookahead, tight_curv;
     float margin;
     uint32_t *n_match;
     float *chi2;
@@ -231,8 +231,8 @@ __global__ void __launch_bounds__(kBlock, FIELD == 0 ? 8 : 0) seed_scan_kernel(c
         // ---- A5: every K steps, the wires near r_n that carry a hit -> slots, with g at this vertex
         if (kcount == 0) {
             // centre of the next K steps (straight-line prediction; the arc's sagitta is in the host's margin); a seed
-            // curling tighter than 20 mm looks up around its own position instead, at the shorter cadence
-            const bool tight = !(fabsf(a) * A.b_max < 0.05f);
+            // curling tighter than that margin allows looks up around its own position instead, at the shorter cadence
+            const bool tight = !(fabsf(a) * A.b_max < A.tight_curv);
             kcount = tight ? A.lookup_every_tight : A.lookup_every;
             const float ahead = tight ? 0.0f : A.lookahead;
             S.n = 0;
@@ -426,7 +426,7 @@ cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0
     A.kq = CDC_KAPPA * (double)L.charge; A.h6_64 = h / 6.0;
     A.kq_rel = (float)(A.kq / (double)(float)A.kq - 1.0);
     A.lambda = L.lambda; A.inv_lambda = 1.0f / L.lambda; A.eloss_h = L.eloss_h; A.window = sqrtf(L.lambda) * 1.0001f;
-    A.u2_lo = L.u2_lo; A.u2_hi = L.u2_hi; A.uz = L.uz; A.inv_uz = L.inv_uz; A.lookup_every = L.lookup_every; A.lookahead = L.lookahead; A.lookup_every_tight = L.lookup_every_tight;
+    A.u2_lo = L.u2_lo; A.u2_hi = L.u2_hi; A.uz = L.uz; A.inv_uz = L.inv_uz; A.lookup_every = L.lookup_every; A.lookahead = L.lookahead; A.lookup_every_tight = L.lookup_every_tight; A.tight_curv = L.tight_curv;
     A.delta_max = L.delta_max; A.b_max = L.b_max; A.hold_path = L.hold_path;
     A.max_steps = L.max_steps; A.margin = L.margin;
     A.n_match = L.d_n_match; A.chi2 = L.d_chi2; A.debug = L.d_debug;

@@ -228,7 +228,7 @@ def test_paper_thread_mapping_gives_the_same_scores(cfg_id):
 
 
 def test_tightly_curling_seeds_use_the_short_lookup_cadence(setup):
-    """Seeds with a track radius below 20 mm (|a| B >= 0.05 / mm) cannot use the look-ahead lookup centre; they fall
+    """Seeds with a small track radius (here below 20 mm) cannot use the look-ahead lookup centre; they fall
     back to a lookup around their own position.  Every wire of the two innermost layers is fired, so any wire the
     candidate set missed would show up as a missing match."""
     cfg, geom, field, events, grids, sc = setup
