@@ -67,7 +67,8 @@ __device__ __forceinline__ void slot_push(Slots &S, int w, float g)
 struct LookupCtx {         // the vertex a lookup is made from
     float x, xl, y, yl, z, Tx, Ty, Tz;     // the vertex itself: g of a new slot is evaluated here
     float cz, phi, g_dead, g_far;          // height and azimuth of the lookup centre
-    float curv, ptol;                      // |a| B_max (0: no pruning by distance, tight curls); window + deviation bound
+    float curv, ptol, hold;                // |a| B_max (0: no pruning by distance, tight curls); window + deviation
+                                           // bound; path to the next lookup
 };
 
 // a candidate with a hit becomes a live slot unless the track has already passed it for good: once g exceeds
@@ -81,12 +82,13 @@ __device__ __forceinline__ void consider(const ScanArgs &A, const uint32_t *s_bi
     const float4 wr = __ldg(A.gd.wire4 + w);
     const float g = wire_g(wr, A.uz, A.inv_uz, V.x, V.xl, V.y, V.yl, V.z, V.Tx, V.Ty, V.Tz, ex, ey, eu);
     if (!(g <= V.g_dead && g > V.g_far)) return;
-    // A wire still ahead (g <= 0) comes no closer to the TANGENT than D0 = sqrt(|delta|^2 - g^2 / |T_w|^2) (T_w: T
-    // without its component along the wire).  After a path t the track is within |a| B t^2 / 2 of its tangent and the
-    // distance to a line is 1-Lipschitz, so an approach owned before the next lookup (t <= K h) has
-    // D0 - dev <= D <= D0 + dev with dev = |a| B (K h)^2 / 2 (the minimum of the true distance over the hold is at
-    // most its value where the tangent is closest).  If the drift circle cannot be met within the window even so,
-    // the wire is not made a live slot.
+    // A wire still ahead (g <= 0) comes no closer to the TANGENT than D0 = sqrt(|delta|^2 - g^2 / |T_w|^2), at the path
+    // s = -g / |T_w|^2 (T_w: T without its component along the wire).  After a path t the track is within
+    // |a| B t^2 / 2 of its tangent and the distance to a line is 1-Lipschitz.  An approach owned before the next lookup
+    // (path t* <= hold = K h) is the one minimum of the true distance over the hold, so
+    //   D >= D0 - dev,  dev = |a| B hold^2 / 2            (the tangent is nowhere closer than D0), and
+    //   D <= D0 + dev  provided s <= hold                 (the true distance at s is a value the minimum cannot exceed).
+    // If the drift circle cannot be met within the window even so, the wire is not made a live slot.
     if (g <= 0.0f && V.curv > 0.0f) {
         const float uT = fmaf(wr.z, V.Tx, fmaf(wr.w, V.Ty, A.uz * V.Tz));
         const float tw2 = fmaf(-uT, uT, 1.0f);
@@ -94,7 +96,8 @@ __device__ __forceinline__ void consider(const ScanArgs &A, const uint32_t *s_bi
             const float D2 = fmaxf(fmaf(-g, g * rcp_normal(tw2), fmaf(ex, ex, fmaf(ey, ey, -eu * eu))), 0.0f);
             const float d = __ldg(drift_e + w);
             const float hi = d + V.ptol, lo = d - V.ptol;
-            if (D2 > hi * hi || (lo > 0.0f && D2 < lo * lo)) return;
+            if (D2 > hi * hi) return;
+            if (lo > 0.0f && D2 < lo * lo && -g <= V.hold * tw2) return;
         }
     }
     slot_push(S, w, g);
@@ -259,6 +262,7 @@ __global__ void __launch_bounds__(kBlock, FIELD == 0 ? 8 : 0) seed_scan_kernel(c
                     V.curv = tight ? 0.0f : (ELOSS ? 1.05f : 1.0f) * fabsf(a) * A.b_max;
                     const float hold = (float)kcount * h + 0.5f;           // path to the next lookup (+ margin)
                     V.ptol = fmaf(0.6f * V.curv, hold * hold, A.window + 0.05f);
+                    V.hold = hold;
                 }
                 lookup_layer(A, s_layer, s_bits, drift_e, jc, V, S, cnt);
                 lookup_layer(A, s_layer, s_bits, drift_e, j2, V, S, cnt);
