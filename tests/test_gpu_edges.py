@@ -251,7 +251,10 @@ def test_tightly_curling_seeds_use_the_short_lookup_cadence(setup):
     bad = np.nonzero((gpu["n_match"] != orc["n_match"]) | (gpu["debug"]["n_steps"] != orc["n_steps"]))[0]
     for i in bad:
         ev = synth.Event(wire_id=w, drift_mm=d, truth_turn=np.zeros_like(w), seed=np.zeros(5), n_turns=1, n_signal=0)
-        assert U.explain_mismatch(bound, ev, g.node(g.unravel(int(i))), cfg, geom2)
+        same = gpu["debug"]["n_steps"][i] == orc["n_steps"][i] and gpu["debug"]["m_gas"][i] == orc["m_gas"][i]
+        assert U.explain_mismatch(bound, ev, g.node(g.unravel(int(i))), cfg, geom2,
+                                  dn=int(gpu["n_match"][i]) - int(orc["n_match"][i]),
+                                  dchi2=float(gpu["chi2"][i]) - float(orc["chi2"][i]), same_track=bool(same))
     assert bad.size <= 3
 
 
@@ -281,7 +284,10 @@ def test_moderately_curling_seeds_dense_hits_every_seed(setup, field_kind):
     bad = np.nonzero((gpu["n_match"] != orc["n_match"]) | (gpu["debug"]["n_steps"] != orc["n_steps"]))[0]
     for i in bad:
         ev = synth.Event(wire_id=w, drift_mm=d, truth_turn=np.zeros_like(w), seed=np.zeros(5), n_turns=1, n_signal=0)
-        assert U.explain_mismatch(bound, ev, g.node(g.unravel(int(i))), cfg2, geom2), int(i)
+        same = gpu["debug"]["n_steps"][i] == orc["n_steps"][i] and gpu["debug"]["m_gas"][i] == orc["m_gas"][i]
+        assert U.explain_mismatch(bound, ev, g.node(g.unravel(int(i))), cfg2, geom2,
+                                  dn=int(gpu["n_match"][i]) - int(orc["n_match"][i]),
+                                  dchi2=float(gpu["chi2"][i]) - float(orc["chi2"][i]), same_track=bool(same)), int(i)
     print(f"field {field_kind}: {bad.size} listed threshold cases of {g.n_seeds} seeds: {bad.tolist()}")
     assert bad.size <= int(1e-2 * g.n_seeds)                  # ~40 approaches per seed here, each with two window edges
     sc2.close()
