@@ -291,3 +291,36 @@ def test_moderately_curling_seeds_dense_hits_every_seed(setup, field_kind):
     print(f"field {field_kind}: {bad.size} listed threshold cases of {g.n_seeds} seeds: {bad.tolist()}")
     assert bad.size <= int(1e-2 * g.n_seeds)                  # ~40 approaches per seed here, each with two window edges
     sc2.close()
+
+
+@pytest.mark.parametrize("field_kind,h,window,steps", [(0, 4.0, 7.0, 750), (1, 0.5, 0.5, 3000), (1, 3.0, 5.0, 1000)])
+def test_every_wire_fired_at_the_corners_of_step_and_window(field_kind, h, window, steps):
+    """All 4512 wires carry a hit with a random drift distance; the largest window the 2 x 2 lookup admits at h = 4 mm
+    (lookup every step), a small step with a narrow window (lookup every 16 steps), and one in between.  Every seed
+    against the oracle; differences must be window-edge cases (chi2 difference = dn * lambda) or track thresholds."""
+    import dataclasses
+    geom = synth.make_geometry()
+    field = synth.make_uniform_field() if field_kind == 0 else synth.make_table_field()
+    rng = np.random.default_rng(23)
+    w = np.arange(0, int(geom.offset[-1]), dtype=np.int32)
+    d = rng.uniform(0.0, 8.0, size=w.size).astype(np.float32)
+    cfg = dataclasses.replace(synth.CONFIGS[1], h_mm=h, window_mm=window, max_steps=steps, field_kind=field_kind)
+    base = synth.generate_events(synth.CONFIGS[1 if field_kind == 0 else 3], geom, field, 1, first_event=7)[0]
+    ev = synth.Event(wire_id=w, drift_mm=d, truth_turn=-np.ones_like(w), seed=base.seed, n_turns=1, n_signal=0)
+    grid = synth.truth_anchored_grid(base.seed, 5)[0]
+    sc = api.SeedScanner(geom, field)
+    E = sc.upload(np.array([0, w.size], dtype=np.int32), w, d)
+    gpu = sc.scan(E, [grid], U.gpu_params(cfg), per_seed=True, debug=True)
+    orc = oracle.scan_parallel(geom, field, U.oracle_params(cfg), w, d, grid)
+    assert orc["n_match"].mean() > 5
+    dbg = gpu["debug"]
+    same = (dbg["n_steps"] == orc["n_steps"]) & (dbg["m_gas"] == orc["m_gas"])
+    bad = np.nonzero((gpu["n_match"] != orc["n_match"]) | ~same)[0]
+    bound = oracle.Bound(geom, field, U.oracle_params(cfg))
+    for i in bad:
+        assert U.explain_mismatch(bound, ev, grid.node(grid.unravel(int(i))), cfg, geom,
+                                  dn=int(gpu["n_match"][i]) - int(orc["n_match"][i]),
+                                  dchi2=float(gpu["chi2"][i]) - float(orc["chi2"][i]), same_track=bool(same[i])), int(i)
+    assert bad.size <= int(5e-3 * grid.n_seeds)
+    U.check_best(cfg, geom, field, ev, grid, gpu, orc_full=orc)
+    sc.close()
