@@ -75,7 +75,8 @@ typedef struct {
 
 /* Propagation and scoring parameters (BJ configs[0]: fixed 2 mm step, <= 1500 steps, 1 mm window).
  * window_mm: a hit matches iff (D - drift)^2 < lambda = window_mm^2  (Eq. (1), reading C9/C10).
- * eloss_MeV_per_mm: constant momentum loss per mm of in-gas path (BJ configs[2], reading C6).
+ * eloss_MeV_per_mm: constant momentum loss per mm of in-gas path (BJ configs[2], reading C6); the scan accepts up to
+ *   ~3e-3 MeV/mm at h = 2 mm (CDC_ERR_RANGE above: its curvature bounds assume < 0.04 MeV/c lost per lookup period).
  * rescore_margin: seeds whose fp32 score is within this of the event's fp32 maximum are re-evaluated in
  * fp64 by cdc_best_track (reading C11); <= 0 selects the default 0.05. */
 typedef struct {

@@ -213,6 +213,10 @@ extern "C" int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cd
         // the track has moved at most K h since: |delta| <= diag + K h; it stays held while the track crosses
         // that neighbourhood, at most ~(diag + K h) / min|T_perp| of path -- bounded here by 4 diag
         const double diag = hypot(2.0 * g->pitch, 2.0 * g->cell_max);
+        // the kernel's curvature bounds allow |a| = kappa / p to grow by 5 % between two lookups; p > 1 MeV/c on a live
+        // track, so the momentum lost over one lookup period must stay below 0.04 MeV/c
+        if (p->eloss_MeV_per_mm * (std::max(K, K0) * p->h_mm + 1.0) > 0.04)
+            CDC_FAIL(CDC_ERR_RANGE, "cdc_seed_scan: energy loss too large for the lookup cadence (eloss * K h must stay below 0.04 MeV/c)");
         L.delta_max = (float)(diag + std::max(K, K0) * p->h_mm + 1.0);
         L.b_max = (float)(1.001 * g->b_max);
         L.hold_path = (float)(4.0 * diag + 2.0 * std::max(K, K0) * p->h_mm);

@@ -61,6 +61,18 @@ def test_upload_errors_are_reported(setup):
     assert ei.value.status == -5
 
 
+def test_energy_loss_beyond_the_curvature_bounds_is_rejected(setup):
+    cfg, geom, field, events, grids, sc = setup
+    off, w, d = synth.pack_hits(events[:1])
+    E = sc.upload(off, w, d)
+    import torch
+    key = torch.zeros(1, dtype=torch.int64, device="cuda")
+    B.cdc_seed_scan(sc.geometry, E, B.grid_specs(grids[:1]), B.scan_params(2.0, 50, 1.0, 2.5e-3), key)     # accepted
+    with pytest.raises(B.CdcError) as ei:
+        B.cdc_seed_scan(sc.geometry, E, B.grid_specs(grids[:1]), B.scan_params(2.0, 50, 1.0, 0.01), key)
+    assert ei.value.status == -2
+
+
 def test_field_table_too_small_is_rejected(setup):
     cfg, geom, *_ = setup
     small = synth.make_table_field(r_max=800.0)
