@@ -42,6 +42,7 @@ void free_geometry(cdc_geometry *g)
 // ------------------------------------------------------------------------------------------------ A0
 extern "C" int32_t cdc_geometry_create(const cdc_geometry_desc *gd, const cdc_field_desc *fd, cdc_geometry **out)
 {
+    return cdc_guard("cdc_geometry_create", [&]() -> int32_t {
     if (!gd || !fd || !out) CDC_FAIL(CDC_ERR_INVALID, "cdc_geometry_create: null argument");
     *out = nullptr;
     const int L = gd->n_layers;
@@ -209,18 +210,23 @@ extern "C" int32_t cdc_geometry_create(const cdc_geometry_desc *gd, const cdc_fi
     q.dr = fd->dr_mm; q.dz = fd->dz_mm; q.tab = (const float *)g->d_field;
     *out = g;
     return CDC_OK;
+    });
 }
 
 extern "C" int32_t cdc_geometry_destroy(cdc_geometry *g)
 {
+    return cdc_guard("cdc_geometry_destroy", [&]() -> int32_t {
     free_geometry(g);
     return CDC_OK;
+    });
 }
 
 extern "C" int32_t cdc_geometry_wire_table(const cdc_geometry *g, float *h_wire, int32_t *n_wires_total)
 {
+    return cdc_guard("cdc_geometry_wire_table", [&]() -> int32_t {
     if (!g) CDC_FAIL(CDC_ERR_INVALID, "cdc_geometry_wire_table: null geometry");
     if (n_wires_total) *n_wires_total = g->W;
     if (h_wire) memcpy(h_wire, g->wire5.data(), sizeof(float) * 5 * (size_t)g->W);
     return CDC_OK;
+    });
 }

@@ -37,6 +37,7 @@ extern "C" int32_t cdc_find_tracks_host(const cdc_geometry *g, int32_t n_events,
                                         double *h_best_chi2, uint64_t *h_best_key, int32_t *h_labels,
                                         double *h_ranges, void *stream)
 {
+    return cdc_guard("cdc_find_tracks_host", [&]() -> int32_t {
     if (!g || !h_hit_offsets || !h_grids || !params || !h_best_seed || !h_best_n_match || !h_best_chi2 || !h_best_key)
         CDC_FAIL(CDC_ERR_INVALID, "cdc_find_tracks_host: null argument");
     if (hp && !h_zref_mm) CDC_FAIL(CDC_ERR_INVALID, "cdc_find_tracks_host: Hough ranges need h_zref_mm");
@@ -87,4 +88,5 @@ extern "C" int32_t cdc_find_tracks_host(const cdc_geometry *g, int32_t n_events,
     if (rc != CDC_OK) return rc;
     if (st.n_pool > st.pool_cap) CDC_FAIL(CDC_ERR_RANGE, "cdc_find_tracks_host: candidate pool overflow");
     return CDC_OK;
+    });
 }

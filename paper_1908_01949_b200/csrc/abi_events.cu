@@ -54,6 +54,7 @@ extern "C" int32_t cdc_event_upload(const cdc_geometry *g, int32_t n_events, con
                                     const int32_t *wire_id, const float *drift_mm, int32_t hits_on_device,
                                     void *stream, cdc_events **out)
 {
+    return cdc_guard("cdc_event_upload", [&]() -> int32_t {
     if (!g || !h_hit_offsets || !out) CDC_FAIL(CDC_ERR_INVALID, "cdc_event_upload: null argument");
     *out = nullptr;
     if (n_events < 1 || n_events > 65535) CDC_FAIL(CDC_ERR_INVALID, "cdc_event_upload: n_events must be in [1, 65535]");
@@ -97,20 +98,25 @@ extern "C" int32_t cdc_event_upload(const cdc_geometry *g, int32_t n_events, con
     if (err & 4) { free_events(ev); CDC_FAIL(CDC_ERR_INVALID, "cdc_event_upload: duplicate wire id within an event"); }
     *out = ev;
     return CDC_OK;
+    });
 }
 
 extern "C" int32_t cdc_events_destroy(cdc_events *ev)
 {
+    return cdc_guard("cdc_events_destroy", [&]() -> int32_t {
     free_events(ev);
     return CDC_OK;
+    });
 }
 
 extern "C" int32_t cdc_events_tables(const cdc_events *ev, float *h_drift_of_wire, uint32_t *h_hit_bits)
 {
+    return cdc_guard("cdc_events_tables", [&]() -> int32_t {
     if (!ev) CDC_FAIL(CDC_ERR_INVALID, "cdc_events_tables: null events");
     if (h_drift_of_wire)
         CDC_CUDA(cudaMemcpy(h_drift_of_wire, ev->d_drift_tab, sizeof(float) * (size_t)ev->n_events * ev->W, cudaMemcpyDeviceToHost));
     if (h_hit_bits)
         CDC_CUDA(cudaMemcpy(h_hit_bits, ev->d_bits, sizeof(uint32_t) * (size_t)ev->n_events * ev->n_bit_words, cudaMemcpyDeviceToHost));
     return CDC_OK;
+    });
 }

@@ -47,6 +47,7 @@ extern "C" int32_t cdc_peel_turns(const cdc_geometry *g, cdc_events *ev, const c
                                   int32_t *h_status, double *h_seeds, uint32_t *h_n_match, double *h_chi2,
                                   double *h_centres_or_null, int32_t *d_partition, void *stream)
 {
+    return cdc_guard("cdc_peel_turns", [&]() -> int32_t {
     if (!g || !ev || !h_grids0 || !p || !pp || !h_n_partitions || !h_status || !h_seeds || !h_n_match || !h_chi2)
         CDC_FAIL(CDC_ERR_INVALID, "cdc_peel_turns: null argument");
     if (ev->geom != g) CDC_FAIL(CDC_ERR_INVALID, "cdc_peel_turns: events belong to another geometry");
@@ -153,4 +154,5 @@ extern "C" int32_t cdc_peel_turns(const cdc_geometry *g, cdc_events *ev, const c
         }
     }
     return CDC_OK;
+    });
 }

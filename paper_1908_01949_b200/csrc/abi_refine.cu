@@ -36,6 +36,7 @@ extern "C" int32_t cdc_refine_tracks(const cdc_geometry *g, cdc_events *ev, cons
                                      int32_t *h_labels_or_null, double *h_trace_S_or_null, int64_t *h_trace_q_or_null,
                                      void *stream)
 {
+    return cdc_guard("cdc_refine_tracks", [&]() -> int32_t {
     if (!g || !ev || !h_grids || !p || !rp || !h_best_seed || !h_best_S || !h_best_n_match || !h_best_chi2 || !h_best_q)
         CDC_FAIL(CDC_ERR_INVALID, "cdc_refine_tracks: null argument");
     if (ev->geom != g) CDC_FAIL(CDC_ERR_INVALID, "cdc_refine_tracks: events belong to another geometry");
@@ -176,4 +177,5 @@ extern "C" int32_t cdc_refine_tracks(const cdc_geometry *g, cdc_events *ev, cons
         CDC_CUDA(cudaStreamSynchronize(s));
     }
     return CDC_OK;
+    });
 }

@@ -126,6 +126,7 @@ int32_t cdc_lookup_every64(const cdc_geometry *g, double h_mm, double window_mm)
 // ------------------------------------------------------------------------------------------------ A2
 extern "C" int32_t cdc_hough_dims(const cdc_hough_params *hp, int32_t *dims3)
 {
+    return cdc_guard("cdc_hough_dims", [&]() -> int32_t {
     if (!hp || !dims3) CDC_FAIL(CDC_ERR_INVALID, "cdc_hough_dims: null argument");
     if (!(hp->bin_xy_mm > 0) || !(hp->bin_R_mm > 0) || !(hp->R_hi_mm > hp->R_lo_mm) || !(hp->half_xy_mm > 0) || !(hp->tol_mm > 0))
         CDC_FAIL(CDC_ERR_INVALID, "cdc_hough_dims: bad Hough parameters");
@@ -135,12 +136,14 @@ extern "C" int32_t cdc_hough_dims(const cdc_hough_params *hp, int32_t *dims3)
     if (dims3[0] < 1 || dims3[1] < 1 || (int64_t)dims3[0] * dims3[1] * dims3[2] > 0x7FFFFFFFLL || dims3[0] > 256)
         CDC_FAIL(CDC_ERR_RANGE, "cdc_hough_dims: accumulator too large (nR <= 256, bins < 2^31)");
     return CDC_OK;
+    });
 }
 
 extern "C" int32_t cdc_hough_seed_ranges(const cdc_geometry *g, const cdc_events *ev, const cdc_hough_params *hp,
                                          int32_t charge, const float *d_zref_mm, double *d_ranges, int32_t *d_peak,
                                          uint32_t *d_accum_or_null, void *stream)
 {
+    return cdc_guard("cdc_hough_seed_ranges", [&]() -> int32_t {
     if (!g || !ev || !hp || !d_zref_mm || !d_ranges || !d_peak) CDC_FAIL(CDC_ERR_INVALID, "cdc_hough_seed_ranges: null argument");
     if (ev->geom != g) CDC_FAIL(CDC_ERR_INVALID, "cdc_hough_seed_ranges: events belong to another geometry");
     if (charge != 1 && charge != -1) CDC_FAIL(CDC_ERR_INVALID, "cdc_hough_seed_ranges: charge must be +-1");
@@ -157,6 +160,7 @@ extern "C" int32_t cdc_hough_seed_ranges(const cdc_geometry *g, const cdc_events
     L.d_ranges = d_ranges; L.d_peak = d_peak; L.d_accum = d_accum_or_null; L.d_peak_key = ev->d_peak_key;
     CDC_CUDA(launch_hough(L, (cudaStream_t)stream));
     return CDC_OK;
+    });
 }
 
 // ------------------------------------------------------------------------------------------------ A3-A7
@@ -164,6 +168,7 @@ extern "C" int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cd
                                  const cdc_scan_params *p, uint32_t *d_n_match, float *d_chi2,
                                  cdc_seed_debug *d_debug, uint64_t *d_best_key, void *stream)
 {
+    return cdc_guard("cdc_seed_scan", [&]() -> int32_t {
     if (!g || !ev || !h_grids || !d_best_key) CDC_FAIL(CDC_ERR_INVALID, "cdc_seed_scan: null argument");
     if (ev->geom != g) CDC_FAIL(CDC_ERR_INVALID, "cdc_seed_scan: events belong to another geometry");
     int32_t rc = check_params(p, "cdc_seed_scan");
@@ -227,10 +232,12 @@ extern "C" int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cd
     CDC_CUDA(launch_seed_scan(L, s, ev->ev_k0, ev->ev_k1));
     ev->scanned = true;
     return CDC_OK;
+    });
 }
 
 extern "C" int32_t cdc_scan_get_stats(const cdc_events *ev, cdc_scan_stats *out, void *stream)
 {
+    return cdc_guard("cdc_scan_get_stats", [&]() -> int32_t {
     if (!ev || !out) CDC_FAIL(CDC_ERR_INVALID, "cdc_scan_get_stats: null argument");
     if (!ev->scanned) CDC_FAIL(CDC_ERR_NOT_READY, "cdc_scan_get_stats: no scan has run on these events");
     unsigned long long c[CNT_N];
@@ -246,6 +253,7 @@ extern "C" int32_t cdc_scan_get_stats(const cdc_events *ev, cdc_scan_stats *out,
     CDC_CUDA(cudaEventElapsedTime(&ms, ev->ev_k0, ev->ev_k1));
     out->kernel_ms = (double)ms;
     return CDC_OK;
+    });
 }
 
 // ------------------------------------------------------------------------------------------------ A8-A9
@@ -253,6 +261,7 @@ extern "C" int32_t cdc_best_track(const cdc_geometry *g, cdc_events *ev, const c
                                   const cdc_scan_params *p, const uint64_t *d_best_key, int64_t *d_best_seed,
                                   uint32_t *d_best_n_match, double *d_best_chi2, int32_t *d_labels, void *stream)
 {
+    return cdc_guard("cdc_best_track", [&]() -> int32_t {
     if (!g || !ev || !h_grids || !d_best_key || !d_best_seed || !d_best_n_match || !d_best_chi2)
         CDC_FAIL(CDC_ERR_INVALID, "cdc_best_track: null argument");
     if (ev->geom != g) CDC_FAIL(CDC_ERR_INVALID, "cdc_best_track: events belong to another geometry");
@@ -277,11 +286,14 @@ extern "C" int32_t cdc_best_track(const cdc_geometry *g, cdc_events *ev, const c
     L.d_best_seed = d_best_seed; L.d_best_n_match = d_best_n_match; L.d_best_chi2 = d_best_chi2; L.d_labels = d_labels;
     CDC_CUDA(launch_best_track(L, (cudaStream_t)stream));
     return CDC_OK;
+    });
 }
 
 extern "C" int32_t cdc_fp32_peak_probe(int32_t iters, double *h_flops_per_s, double *h_ms, void *stream)
 {
+    return cdc_guard("cdc_fp32_peak_probe", [&]() -> int32_t {
     if (iters < 1) CDC_FAIL(CDC_ERR_INVALID, "cdc_fp32_peak_probe: iters < 1");
     CDC_CUDA(run_fp32_peak_probe(iters, h_flops_per_s, h_ms, (cudaStream_t)stream));
     return CDC_OK;
+    });
 }

@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <new>
+#include <stdexcept>
 #include <string>
 #include <vector>
 
@@ -155,6 +157,23 @@ void cdc_set_error(const std::string &msg);
 #define CDC_CUDA(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { \
     cdc_set_error(std::string(#expr) + ": " + cudaGetErrorString(e_)); \
     return (e_ == cudaErrorMemoryAllocation) ? CDC_ERR_NOMEM : CDC_ERR_CUDA; } } while (0)
+
+// ---- no exception crosses the C boundary (include/cdc_seedscan.h): every int32_t entry point runs inside this
+template <typename F>
+inline int32_t cdc_guard(const char *who, F &&body) noexcept
+{
+    try {
+        return body();
+    } catch (const std::bad_alloc &) {
+        try { cdc_set_error(std::string(who) + ": out of host memory"); } catch (...) {}
+        return CDC_ERR_NOMEM;
+    } catch (const std::exception &e) {
+        try { cdc_set_error(std::string(who) + ": " + e.what()); } catch (...) {}
+        return CDC_ERR_INVALID;
+    } catch (...) {
+        return CDC_ERR_INVALID;
+    }
+}
 
 // ---- launchers implemented in the kernel translation units ---------------------------------------
 struct ScanLaunch {

@@ -52,6 +52,7 @@ extern "C" int32_t cdc_seed_scan_paper_mapping(const cdc_geometry *g, cdc_events
                                                const cdc_scan_params *p, const int64_t *d_seed_index, int32_t n_seeds,
                                                uint32_t *d_n_match, float *d_chi2, void *stream)
 {
+    return cdc_guard("cdc_seed_scan_paper_mapping", [&]() -> int32_t {
     cudaStream_t s = (cudaStream_t)stream;
     PaperArgs A;
     double *d_axes = nullptr;
@@ -66,4 +67,5 @@ extern "C" int32_t cdc_seed_scan_paper_mapping(const cdc_geometry *g, cdc_events
     cudaFreeAsync(d_axes, s);
     CDC_CUDA(e);
     return CDC_OK;
+    });
 }

@@ -79,6 +79,7 @@ extern "C" int32_t cdc_seed_scan_paper_mapping_v2(const cdc_geometry *g, cdc_eve
                                                   const int64_t *d_seed_index, int32_t n_seeds, uint32_t *d_n_match,
                                                   float *d_chi2, double *h_ms2_or_null, void *stream)
 {
+    return cdc_guard("cdc_seed_scan_paper_mapping_v2", [&]() -> int32_t {
     cudaStream_t s = (cudaStream_t)stream;
     PaperArgs A;
     double *d_axes = nullptr;
@@ -121,4 +122,5 @@ extern "C" int32_t cdc_seed_scan_paper_mapping_v2(const cdc_geometry *g, cdc_eve
     cudaFreeAsync(d_axes, s);
     CDC_CUDA(e);
     return CDC_OK;
+    });
 }

@@ -62,6 +62,7 @@ extern "C" int32_t cdc_classification_quality(const cdc_events *ev, int32_t n_tu
                                               const int32_t *d_truth_turn, int32_t *d_confusion, int32_t *d_c_true,
                                               int32_t *d_noise_into, double *d_efficiency, double *d_purity, void *stream)
 {
+    return cdc_guard("cdc_classification_quality", [&]() -> int32_t {
     if (!ev || !d_labels || !d_truth_turn || !d_confusion || !d_c_true || !d_noise_into || !d_efficiency || !d_purity)
         CDC_FAIL(CDC_ERR_INVALID, "cdc_classification_quality: null argument");
     if (n_turns < 1 || n_turns > kMaxTurns) CDC_FAIL(CDC_ERR_INVALID, "cdc_classification_quality: n_turns must be in [1, 8]");
@@ -70,14 +71,17 @@ extern "C" int32_t cdc_classification_quality(const cdc_events *ev, int32_t n_tu
     cdc_count_launch();
     CDC_CUDA(cudaGetLastError());
     return CDC_OK;
+    });
 }
 
 extern "C" int32_t cdc_common_hits(const cdc_events *ev, const int32_t *d_labels_a, const int32_t *d_labels_b,
                                    int32_t turn_a, int32_t turn_b, int32_t *d_n_common, void *stream)
 {
+    return cdc_guard("cdc_common_hits", [&]() -> int32_t {
     if (!ev || !d_labels_a || !d_labels_b || !d_n_common) CDC_FAIL(CDC_ERR_INVALID, "cdc_common_hits: null argument");
     common_kernel<<<ev->n_events, 256, 0, (cudaStream_t)stream>>>(ev->d_offsets, d_labels_a, d_labels_b, turn_a, turn_b, d_n_common);
     cdc_count_launch();
     CDC_CUDA(cudaGetLastError());
     return CDC_OK;
+    });
 }
