@@ -248,6 +248,44 @@ def test_score_identity_E_equals_lambda_N_minus_S(geom, uniform_field):
         assert res["n_match"] == int((d2 < lam).sum())
 
 
+@pytest.mark.parametrize("cfg_id", [1, 2])
+def test_score_is_eq1_taken_literally_per_turn_partition(geom, uniform_field, cfg_id):
+    """Eq. (1) sums over WIRES: E = sum_w min(d_L^2, d_R^2, lambda), one term per fired wire, for the
+    turn partition under investigation.  The oracle sums over matched APPROACHES and runs through every turn (reading
+    C9: a hit matched in two turns counts in both -- Eq. (1) once per partition).  Written out literally -- per
+    partition t, per fired wire, the SMALLEST d^2 over that wire's approaches in t, a wire never approached in t
+    contributing lambda -- E_total = lambda (n_partitions N_hits - S) must give the oracle's S.  The two differ only if
+    one wire owns two matched approaches within ONE partition; within one passage of the gas the distance to a wire has
+    a single minimum (a circle and a point), so that count is zero on multi-turn seeds of 3000 / 4500 steps."""
+    cfg = synth.CONFIGS[cfg_id]
+    evs = synth.generate_events(cfg, geom, uniform_field, 2)
+    b = _bound(geom, uniform_field, cfg.h_mm, cfg.max_steps, cfg.window_mm, cfg.eloss_MeV_per_mm)
+    lam = cfg.window_mm ** 2
+    rng = np.random.default_rng(11 + cfg_id)
+    multi_turn_repeats = 0
+    for ev in evs:
+        N = ev.wire_id.size
+        for trial in range(12):
+            seed = ev.seed + (0.0 if trial == 0 else 1.0) * rng.uniform(-1, 1, 5) * synth.HALF_WIDTH
+            res = oracle.eval_seed(b, ev.wire_id, ev.drift_mm, seed, mode=0, records=True, rec_slack=1e9)
+            rec = res["rec"]
+            d2 = np.where(np.abs(rec["zw"]) <= 750.0, rec["resid"] ** 2, np.inf)
+            n_part = res["turns"] + 1
+            E = 0.0
+            for t in range(n_part):
+                best = np.full(N, np.inf)                      # per fired wire: min over its approaches in partition t
+                sel = rec["turn"] == t
+                np.minimum.at(best, rec["hit"][sel], d2[sel])
+                E += np.minimum(best, lam).sum()
+                hits_t, counts = np.unique(rec["hit"][sel & (d2 < lam)], return_counts=True)
+                assert counts.size == 0 or counts.max() == 1   # no wire matched twice within one partition
+            S = res["n_match"] - res["chi2"] / lam
+            assert abs(E - lam * (n_part * N - S)) < 1e-9
+            m = rec[d2 < lam]
+            multi_turn_repeats += m.size - np.unique(m["hit"]).size
+    assert multi_turn_repeats > 0      # the cross-partition repeats the reading is about do occur in this sample
+
+
 def test_d_left_right_reading(geom):
     """min(d_L^2, d_R^2) with the two hit positions at +-drift from the wire equals (D - drift)^2 (reading C9)."""
     D = np.linspace(0.0, 9.0, 50); x = 3.3
@@ -329,6 +367,12 @@ def test_turn_counter_and_termination(geom, uniform_field):
     # step cap
     b2 = _bound(geom, uniform_field, 2.0, 37)
     assert oracle.eval_seed(b2, hit_w, drift, seed)["n_steps"] == 37
+    # the turn index counts OUTWARD crossings of R0 (reading C7): a track capped inside R0 after its first gas passage
+    # has left the gas once and re-entered it never -> turns = 0 (counting inward crossings instead would give 1)
+    first_in = int(np.argmax(~gas))                                      # first vertex back inside R0
+    assert first_in > 100 and not gas[first_in + 5]
+    b3 = _bound(geom, uniform_field, 2.0, first_in + 5)
+    assert oracle.eval_seed(b3, hit_w, drift, seed)["turns"] == 0
     # outer wall: a stiff track leaves through r_out
     seed2 = np.array([0.0, 0.0, 400.0, 0.0, 1.0])
     r2 = oracle.eval_seed(b, hit_w, drift, seed2)
