@@ -78,7 +78,11 @@ typedef struct {
  * eloss_MeV_per_mm: constant momentum loss per mm of in-gas path (BJ configs[2], reading C6); the scan accepts up to
  *   ~3e-3 MeV/mm at h = 2 mm (CDC_ERR_RANGE above: its curvature bounds assume < 0.04 MeV/c lost per lookup period).
  * rescore_margin: seeds whose fp32 score is within this of the event's fp32 maximum are re-evaluated in
- * fp64 by cdc_best_track (reading C11); <= 0 selects the default 0.05. */
+ * fp64 by cdc_best_track (reading C11); <= 0 selects the default 0.05.
+ * kernel_variant: 0 = the production kernel (one seed per thread; (x, y) components as packed fp32 pairs);
+ *   1 = two z0-neighbour seeds per thread, every quantity a packed pair of the two seeds (csrc/scan_pair.cu): measured
+ *   slower on B200 (profiles/r2_pair_kernel.md), kept as the comparison point; per-seed n_match,
+ *   step counts, best seed and labels are identical, tests/test_gpu_pair.py checks it. */
 typedef struct {
     double h_mm;
     int32_t max_steps;
@@ -86,6 +90,7 @@ typedef struct {
     double eloss_MeV_per_mm;
     int32_t charge;                          /* -1 for e-  */
     double rescore_margin;
+    int32_t kernel_variant;
 } cdc_scan_params;
 
 /* Hough circle vote (Fig. 4; parametrisation is reading C13): accumulator over circle

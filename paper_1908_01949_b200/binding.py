@@ -45,7 +45,8 @@ class GridSpec(C.Structure):
 
 class ScanParams(C.Structure):
     _fields_ = [("h_mm", C.c_double), ("max_steps", C.c_int32), ("window_mm", C.c_double),
-                ("eloss_MeV_per_mm", C.c_double), ("charge", C.c_int32), ("rescore_margin", C.c_double)]
+                ("eloss_MeV_per_mm", C.c_double), ("charge", C.c_int32), ("rescore_margin", C.c_double),
+                ("kernel_variant", C.c_int32)]
 
 
 class HoughParams(C.Structure):
@@ -117,9 +118,9 @@ def _stream(stream) -> C.c_void_p:
 
 
 def scan_params(h_mm: float, max_steps: int, window_mm: float = 1.0, eloss_MeV_per_mm: float = 0.0,
-                charge: int = -1, rescore_margin: float = 0.0) -> ScanParams:
+                charge: int = -1, rescore_margin: float = 0.0, kernel_variant: int = 0) -> ScanParams:
     return ScanParams(float(h_mm), int(max_steps), float(window_mm), float(eloss_MeV_per_mm), int(charge),
-                      float(rescore_margin))
+                      float(rescore_margin), int(kernel_variant))
 
 
 def hough_params(**kw) -> HoughParams:

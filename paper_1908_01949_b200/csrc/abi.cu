@@ -172,8 +172,10 @@ extern "C" int32_t cdc_geometry_create(const cdc_geometry_desc *gd, const cdc_fi
     if (fd->kind == 1) {
         G_CUDA(dev_alloc(&g->d_field, (size_t)fd->nr * fd->nz));
         G_CUDA(cudaMemcpy(g->d_field, g->field_tab.data(), sizeof(float2) * (size_t)fd->nr * fd->nz, cudaMemcpyHostToDevice));
-        // per-cell bilinear coefficients for the fp32 scan: B(wr, wz) = c0 + c_r wr + c_z wz + c_rz wr wz
-        // (differences of the fp32 node values taken in fp64, rounded once)
+        // per-cell bilinear coefficients for the fp32 scan, taken about the CELL CENTRE:
+        //   B(wr, wz) = c0 + c_r wr + c_z wz + c_rz wr wz,  wr, wz in [-1/2, 1/2] = offset from the centre in cell units
+        // (combinations of the fp32 node values formed in fp64, rounded once), stored as (c0, c_z, c_r, c_rz): the two
+        // register pairs of one 128-bit load are then the operands of ONE packed FMA, (c0, c_z) + wr (c_r, c_rz)
         const int ncr = fd->nr - 1, ncz = fd->nz - 1;
         std::vector<float4> cells((size_t)ncr * ncz * 2);
         for (int iz = 0; iz < ncz; ++iz)
@@ -183,8 +185,10 @@ extern "C" int32_t cdc_geometry_create(const cdc_geometry_desc *gd, const cdc_fi
                     const double n01 = g->field_tab[((size_t)iz * fd->nr + ir + 1) * 2 + c];
                     const double n10 = g->field_tab[((size_t)(iz + 1) * fd->nr + ir) * 2 + c];
                     const double n11 = g->field_tab[((size_t)(iz + 1) * fd->nr + ir + 1) * 2 + c];
+                    const double crz = n11 - n10 - n01 + n00;
                     cells[((size_t)iz * ncr + ir) * 2 + c] =
-                        make_float4((float)n00, (float)(n01 - n00), (float)(n10 - n00), (float)(n11 - n10 - n01 + n00));
+                        make_float4((float)(0.25 * (n00 + n01 + n10 + n11)), (float)((n10 - n00) + 0.5 * crz),
+                                    (float)((n01 - n00) + 0.5 * crz), (float)crz);
                 }
         G_CUDA(dev_alloc(&g->d_cells, cells.size()));
         G_CUDA(cudaMemcpy(g->d_cells, cells.data(), sizeof(float4) * cells.size(), cudaMemcpyHostToDevice));
@@ -201,8 +205,8 @@ extern "C" int32_t cdc_geometry_create(const cdc_geometry_desc *gd, const cdc_fi
     f.kind = fd->kind; f.bz = (float)fd->bz_T; f.nr = fd->nr; f.nz = fd->nz;
     f.r0 = (float)fd->r0_mm; f.z0 = (float)fd->z0_mm;
     f.inv_dr = fd->kind == 1 ? (float)(1.0 / fd->dr_mm) : 0.f; f.inv_dz = fd->kind == 1 ? (float)(1.0 / fd->dz_mm) : 0.f;
-    f.tab = g->d_field; f.cells = g->d_cells;
-    f.cr = fd->kind == 1 ? (float)(-fd->r0_mm / fd->dr_mm) : 0.f; f.cz = fd->kind == 1 ? (float)(-fd->z0_mm / fd->dz_mm) : 0.f;
+    f.tab = g->d_field; f.cells = g->d_cells; f.n_cells = fd->kind == 1 ? (fd->nr - 1) * (fd->nz - 1) : 0;
+    f.cr = fd->kind == 1 ? (float)(-fd->r0_mm / fd->dr_mm - 0.5) : 0.f; f.cz = fd->kind == 1 ? (float)(-fd->z0_mm / fd->dz_mm - 0.5) : 0.f;
     Geom64 &q = g->g64;
     q.n_layers = L; q.n_wires_total = g->W; q.R0 = g->R0; q.z_half = g->z_half; q.r_out = g->r_out;
     q.wire5 = g->d_wire5; q.layers = g->d_layers; q.r_first = d.r_first; q.inv_pitch = d.inv_pitch; q.tan_abs = d.tan_abs;

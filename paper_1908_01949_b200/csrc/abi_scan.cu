@@ -49,6 +49,7 @@ int32_t check_params(const cdc_scan_params *p, const char *who)
     if (!(p->window_mm > 0.0)) CDC_FAIL(CDC_ERR_INVALID, std::string(who) + ": window <= 0");
     if (!(p->eloss_MeV_per_mm >= 0.0)) CDC_FAIL(CDC_ERR_INVALID, std::string(who) + ": negative energy loss");
     if (p->charge != 1 && p->charge != -1) CDC_FAIL(CDC_ERR_INVALID, std::string(who) + ": charge must be +-1");
+    if (p->kernel_variant != 0 && p->kernel_variant != 1) CDC_FAIL(CDC_ERR_INVALID, std::string(who) + ": kernel_variant must be 0 or 1");
     return CDC_OK;
 }
 
@@ -210,9 +211,22 @@ extern "C" int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cd
             const double Kh = K * p->h_mm;
             L.tight_curv = (float)(ahead > 0.0 ? std::min(0.05, 0.98 * 2.0 * sqrt(sag * sag + 2.0 * sag * ahead) / (Kh * Kh)) : 0.05);
         }
-        const double grow = reach + 0.2 + std::max(ahead + sag, (K0 - 1) * p->h_mm);
+        // the two-seed kernel looks wires up around the midpoint of its two seeds, at most sep_cap (as a wire sees it)
+        // from either seed's own centre: every bound that speaks of "the lookup centre" is widened by it
+        const bool pair = p->kernel_variant == 1 && !(g->field.kind != 0 && p->eloss_MeV_per_mm > 0.0);
+        const double sep_cap = pair ? 1.5 : 0.0;
+        L.sep_cap = (float)sep_cap;
+        L.k_margin = (float)(0.9999 * (g->excl - reach - sag) - 0.01);
+        L.k_margin0 = (float)(0.9999 * (g->excl - reach) - 0.01);
+        {
+            double se = 0.0;
+            for (int j = 0; j < g->n_layers; ++j) se = std::max(se, fabs(sin(g->stereo[j])));
+            L.sin_eps = (float)(1.0001 * se);
+        }
+        const double grow = reach + 0.2 + sep_cap + std::max(ahead + sag, (K0 - 1) * p->h_mm);
         const double ulo = std::max(g->r[0] - grow, 0.0), uhi = g->r[g->n_layers - 1] + grow;
         L.u2_lo = (float)(ulo * ulo); L.u2_hi = (float)(uhi * uhi);
+        L.back = (float)(std::max(ahead + 0.2, (K0 - 1) * p->h_mm) + sep_cap);
         L.uz = g->uz; L.inv_uz = (float)(1.0 / (double)g->uz);
         // a held wire lies within the 2 x 2 set of the last lookup vertex (two layer pitches x two cells) and
         // the track has moved at most K h since: |delta| <= diag + K h; it stays held while the track crosses
@@ -222,12 +236,17 @@ extern "C" int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cd
         // track, so the momentum lost over one lookup period must stay below 0.04 MeV/c
         if (p->eloss_MeV_per_mm * (std::max(K, K0) * p->h_mm + 1.0) > 0.04)
             CDC_FAIL(CDC_ERR_RANGE, "cdc_seed_scan: energy loss too large for the lookup cadence (eloss * K h must stay below 0.04 MeV/c)");
-        L.delta_max = (float)(diag + std::max(K, K0) * p->h_mm + 1.0);
+        L.delta_max = (float)(diag + std::max(K, K0) * p->h_mm + 1.0 + sep_cap);
         L.b_max = (float)(1.001 * g->b_max);
-        L.hold_path = (float)(4.0 * diag + 2.0 * std::max(K, K0) * p->h_mm);
+        L.hold_path = (float)(4.0 * diag + 2.0 * std::max(K, K0) * p->h_mm + 2.0 * sep_cap);
     }
     L.max_seeds_per_event = 0;
-    for (const GridDev &G : ev->h_grids) L.max_seeds_per_event = std::max<int64_t>(L.max_seeds_per_event, G.n_seeds);
+    L.max_pairs_per_event = 0;
+    for (const GridDev &G : ev->h_grids) {
+        L.max_seeds_per_event = std::max<int64_t>(L.max_seeds_per_event, G.n_seeds);
+        L.max_pairs_per_event = std::max<int64_t>(L.max_pairs_per_event, ((int64_t)G.n_seeds / G.n[1]) * ((G.n[1] + 1) / 2));
+    }
+    L.variant = p->kernel_variant;
     if (!ev->ev_k0) { CDC_CUDA(cudaEventCreate(&ev->ev_k0)); CDC_CUDA(cudaEventCreate(&ev->ev_k1)); }
     CDC_CUDA(launch_seed_scan(L, s, ev->ev_k0, ev->ev_k1));
     ev->scanned = true;

@@ -32,9 +32,10 @@ struct FieldDev {
     float bz;                // uniform field
     int32_t nr, nz;
     float r0, z0, inv_dr, inv_dz;
-    float cr, cz;            // -r0 / dr, -z0 / dz: cell coordinate = fma(rho, inv_dr, cr)
+    float cr, cz;            // -r0 / dr - 1/2, -z0 / dz - 1/2: fma(rho, inv_dr, cr) = cell coordinate - 1/2
+    int32_t n_cells;         // (nr - 1) (nz - 1)
     const float2 *tab;       // [nz][nr] (B_r, B_z) nodes (fp64 path)
-    const float4 *cells;     // [nz-1][nr-1][2]: bilinear coefficients (c0, c_r, c_z, c_rz) of B_r, then of B_z
+    const float4 *cells;     // [nz-1][nr-1][2]: bilinear coefficients about the cell centre (c0, c_z, c_r, c_rz) of B_r, then of B_z
 };
 
 struct GeomDev {
@@ -197,12 +198,17 @@ struct ScanLaunch {
     uint32_t pool_cap;
     unsigned long long *d_counters;
     int64_t max_seeds_per_event;
+    int64_t max_pairs_per_event;     // two-seeds-per-thread kernel: ceil(n_z / 2) * n_theta * n_px * n_py * n_pz
+    int32_t variant;                 // 0: one seed per thread (scan.cu); 1: two seeds per thread (scan_pair.cu)
     float u2_lo, u2_hi, uz, inv_uz;  // lookup band (widened for the lookup cadence), cos(eps)
     int32_t lookup_every;            // K: steps per layer/cell lookup
     float lookahead;                 // the lookup is centred on r_n + lookahead * T_n (the middle of the next K steps)
     int32_t lookup_every_tight;      // K for tightly curling seeds: lookup centred on r_n itself
+    float back;                      // how far inside the band's lower edge a held wire can still be scored from
     float tight_curv;                // |a| B_max at and above which a seed counts as tightly curling (host: sagitta margin)
     float delta_max, b_max, hold_path;   // largest |delta| of a held wire, largest |B|, longest path a wire stays held
+    float k_margin, k_margin0, sin_eps, sep_cap;  // two-seed kernel: excl - reach - sag, excl - reach (rounded down), sin|stereo|,
+                                         // largest half-separation (as a wire sees it) served by one shared lookup
 };
 cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0, cudaEvent_t k1);
 

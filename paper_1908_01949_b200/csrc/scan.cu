@@ -17,39 +17,10 @@
 // sign change.  Lanes of a warp are seeds that differ in z0 first: they cross the same wires together.
 #include "cdc_internal.cuh"
 #include "scan_common.cuh"
+#include "scan_args.cuh"
+#include "pair_math.cuh"
 
 namespace {
-
-constexpr int kBlock = 128;
-constexpr int kMaxBitWords = 256;          // 8192 wires
-
-struct ScanArgs {
-    GeomDev gd;
-    FieldDev fd;
-    const GridDev *grids;
-    const double *axes;
-    int32_t axis_stride;
-    const float *drift_tab;
-    const uint32_t *bits;
-    float h, h_half, h2_8, h2_2, h_6, h2_6;
-    double kq;                 // kappa * charge
-    float kq_rel;              // kq / fl32(kq) - 1: the systematic part of a = fl32(kq) / p (energy-loss path)
-    double h6_64;              // h / 6 in fp64 (for the systematic-rounding correction)
-    float lambda, inv_lambda, eloss_h, window;
-    float u2_lo, u2_hi;        // lookup band in u^2, widened by (K - 1) h
-    float uz, inv_uz;          // cos(eps) of the canonical wire table (one |stereo| for all layers)
-    float delta_max, b_max, hold_path;   // bounds behind g_dead (see consider())
-    int32_t max_steps, lookup_every, lookup_every_tight;
-    float lookahead, tight_curv;
-    float margin;
-    uint32_t *n_match;
-    float *chi2;
-    cdc_seed_debug *debug;
-    unsigned long long *best_key;
-    PoolEntry *pool;
-    uint32_t pool_cap;
-    unsigned long long *counters;
-};
 
 struct Slots {             // live candidate wires of this thread (those that carry a hit), and g at the current vertex
     int w0, w1, w2, w3;
@@ -122,27 +93,43 @@ __device__ __forceinline__ void lookup_layer(const ScanArgs &A, const LayerDev *
     consider(A, s_bits, drift_e, L.offset + k2, V, S, cnt);
 }
 
-struct Vtx {               // position part of a step vertex (hi + the lo of x, y that the wire offset uses)
-    float x, xl, y, yl, z;
+struct Vtx {               // position part of a step vertex: (x, y) and the lo parts the wire offset uses, as pairs
+    f2 xy, xyl;
+    float z;
 };
+
+// g = delta . T for wire wr = (w0x, w0y, ux, uy) at a vertex: wire_g() of scan_common.cuh with the two horizontal
+// components of e carried as ONE packed pair (the register pairs of the 128-bit wire load are its operands).  Every
+// half rounds like the scalar operation and the order is the same, so the value is bit-identical to wire_g().
+__device__ __forceinline__ float wire_gp(const float4 wr, float uz, float inv_uz, f2 xy, f2 xyl, float z, f2 Txy, float Tz,
+                                         f2 &exy, float &eu)
+{
+    const float zt = __fmul_rn(z, inv_uz);
+    exy = add2(fma2(bc(-zt), pk(wr.z, wr.w), sub2(xy, pk(wr.x, wr.y))), xyl);
+    const float Tx = lo(Txy), Ty = hi(Txy), ex = lo(exy), ey = hi(exy);
+    const float uT = __fmaf_rn(wr.z, Tx, __fmaf_rn(wr.w, Ty, __fmul_rn(uz, Tz)));
+    eu = __fmaf_rn(ex, wr.z, __fmul_rn(ey, wr.w));
+    return __fmaf_rn(ex, Tx, __fmaf_rn(ey, Ty, -__fmul_rn(eu, uT)));
+}
 
 // One live wire over interval n: g at the far vertex; on g_n <= 0 < g_{n+1} the interval owns an approach (C9).
 __device__ __forceinline__ void slot_step(const ScanArgs &A, const float *drift_e, int w, float &g, bool score,
-                                          float sdx, float sdy, float sdz, const Vtx &v1, float Tx1, float Ty1, float Tz1,
+                                          f2 sdxy, float sdz, const Vtx &v1, f2 Txy1, float Tz1,
                                           uint32_t &nm, float &chi2, uint32_t &cnt)
 {
     const float4 wr = __ldg(A.gd.wire4 + w);
-    float ex1, ey1, eu1;
-    const float gn = wire_g(wr, A.uz, A.inv_uz, v1.x, v1.xl, v1.y, v1.yl, v1.z, Tx1, Ty1, Tz1, ex1, ey1, eu1);
+    f2 exy1;
+    float eu1;
+    const float gn = wire_gp(wr, A.uz, A.inv_uz, v1.xy, v1.xyl, v1.z, Txy1, Tz1, exy1, eu1);
     if (score && g <= 0.0f && gn > 0.0f) {
         cnt += 1u << 16;
         // chord point P = r_{n+1} - (1 - tau)(r_{n+1} - r_n): e is linear in the position, and r_{n+1} - r_n is the
         // increment (sdx, sdy, sdz) this step has just added, so e(P) follows from e_{n+1} without the old vertex
         const float zd = sdz * A.inv_uz;
-        const float dex = fmaf(-zd, wr.z, sdx), dey = fmaf(-zd, wr.w, sdy);
+        const f2 dexy = fma2(bc(-zd), pk(wr.z, wr.w), sdxy);
         const float sm = __fdividef(g, g - gn) - 1.0f;         // tau - 1, in [-1, 0)
-        const float ex = fmaf(sm, dex, ex1);
-        const float ey = fmaf(sm, dey, ey1);
+        const f2 exy = fma2(bc(sm), dexy, exy1);
+        const float ex = lo(exy), ey = hi(exy);
         const float eu = fmaf(ex, wr.z, ey * wr.w);
         const float D2 = fmaf(ex, ex, fmaf(ey, ey, -eu * eu));
         const float D = sqrtf(fmaxf(D2, 0.0f));
@@ -155,11 +142,42 @@ __device__ __forceinline__ void slot_step(const ScanArgs &A, const float *drift_
     g = gn;
 }
 
+// tabulated field at (x, y, z): field_at<1>() of scan_common.cuh with (B_x, B_y), the two cell coordinates and the two
+// halves of each bilinear form carried as packed pairs (same operations, same rounding)
+__device__ __forceinline__ void field_at_p(const FieldDev &F, f2 xy, float z, f2 &Bxy, float &Bz)
+{
+    const float x = lo(xy), y = hi(xy);
+    const float rho2 = fmaf(x, x, y * y);
+    const float inv_rho = rsqrt_normal(fmaxf(rho2, 1e-30f));
+    const float rho = rho2 * inv_rho;
+    const f2 f = pk(fmaf(rho, F.inv_dr, F.cr), fmaf(z, F.inv_dz, F.cz));          // (r, z) cell coordinates - 1/2
+    const f2 t = add2(f, kMagicRound);
+    const f2 w = sub2(f, sub2(t, kMagicRound));                                     // offsets from the cell centre
+    const int ir = __float_as_int(lo(t)) - kMagicRoundBits, iz = __float_as_int(hi(t)) - kMagicRoundBits;
+    const unsigned cell = min((unsigned)(iz * (F.nr - 1) + ir), (unsigned)(F.n_cells - 1));
+    const float4 *c = F.cells + 2u * cell;
+    const float4 cr = __ldg(c), cz = __ldg(c + 1);                                  // (c0, c_z, c_r, c_rz) of B_r, of B_z
+    const f2 tr = fma2(bc(lo(w)), pk(cr.z, cr.w), pk(cr.x, cr.y)), tz = fma2(bc(lo(w)), pk(cz.z, cz.w), pk(cz.x, cz.y));
+    const float Br = fmaf(hi(w), hi(tr), lo(tr));
+    Bz = fmaf(hi(w), hi(tz), lo(tz));
+    Bxy = mul2(bc(Br * inv_rho), xy);
+}
+
 // TRACK: keep the in-gas flag, the in-gas step count and the turn counter.  They are needed with energy loss (p_n is
 // defined through m_n), for the debug record, and when a held wire could be scored from a vertex inside R0; otherwise
 // every vertex a wire can be scored from lies in the gas (host check in launch_seed_scan) and they are dead weight.
+#ifndef SCAN_UNROLL
+#define SCAN_UNROLL 2
+#endif
+constexpr int kScanUnroll = SCAN_UNROLL;     // main loop unroll factor
+#ifndef SCAN_MB0
+#define SCAN_MB0 8           // resident blocks per SM the uniform-field variants are held to (64 registers)
+#endif
+#ifndef SCAN_MB1
+#define SCAN_MB1 0
+#endif
 template <int FIELD, bool ELOSS, bool TRACK>
-__global__ void __launch_bounds__(kBlock, FIELD == 0 ? 8 : 0) seed_scan_kernel(const ScanArgs A)
+__global__ void __launch_bounds__(kBlock, FIELD == 0 ? SCAN_MB0 : SCAN_MB1) seed_scan_kernel(const ScanArgs A)
 {
     __shared__ LayerDev s_layer[CDC_MAX_LAYERS];
     __shared__ uint32_t s_bits[kMaxBitWords];
@@ -187,9 +205,13 @@ __global__ void __launch_bounds__(kBlock, FIELD == 0 ? 8 : 0) seed_scan_kernel(c
     const int i_pz = q / G.n[3];
     const uint32_t index = (uint32_t)((((i_th * G.n[1] + i_z) * G.n[2] + i_px) * G.n[3] + i_py) * G.n[4] + i_pz);
 
-    float xh, xl, yh, yl, zh, zl, Txh, Txl, Tyh, Tyl, Tzh, Tzl, a, epsT, p0h, p0l;
+    // state: (x, y) and (Tx, Ty) as packed pairs (one FFMA2 / FADD2 serves both components), z and Tz scalar; every
+    // component hi + lo (compensated)
+    f2 xyh, xyl, Txyh, Txyl;
+    float zh, zl, Tzh, Tzl, a, epsT, p0h, p0l;
     float ub_h = 0.f, ub_l = 0.f, ue1 = 0.f, up1 = 0.f, up2_h = 0.f, up2_l = 0.f;   // uniform-field step map (FIELD == 0)
     {
+        float xh, xl, yh, yl, Txh, Txl, Tyh, Tyl;
         const double *ax = A.axes + (size_t)e * 6 * A.axis_stride;
         double x0 = ax[i_th], y0 = ax[A.axis_stride + i_th], z0 = ax[2 * A.axis_stride + i_z];
         double px = ax[3 * A.axis_stride + i_px], py = ax[4 * A.axis_stride + i_py], pz = ax[5 * A.axis_stride + i_pz];
@@ -216,6 +238,7 @@ __global__ void __launch_bounds__(kBlock, FIELD == 0 ? 8 : 0) seed_scan_kernel(c
             ue1 = (float)(-th2 / 2.0 + th2 * th2 / 24.0);
             up1 = (float)(-h64 * th2 / 6.0);
         }
+        xyh = pk(xh, yh); xyl = pk(xl, yl); Txyh = pk(Txh, Tyh); Txyl = pk(Txl, Tyl);
     }
     // p <= 1 MeV/c ends a track after its first step (C7)
     // (a thread beyond the grid takes no step: its `valid` folded into the step cap keeps the loop test to one compare)
@@ -229,7 +252,7 @@ __global__ void __launch_bounds__(kBlock, FIELD == 0 ? 8 : 0) seed_scan_kernel(c
     Slots S;
     S.n = 0; S.w0 = S.w1 = S.w2 = S.w3 = 0; S.g0 = S.g1 = S.g2 = S.g3 = 0.0f;
 
-#pragma unroll 2
+#pragma unroll kScanUnroll
     while (n < max_steps) {
         // ---- A5: every K steps, the wires near r_n that carry a hit -> slots, with g at this vertex
         if (kcount == 0) {
@@ -239,6 +262,7 @@ __global__ void __launch_bounds__(kBlock, FIELD == 0 ? 8 : 0) seed_scan_kernel(c
             kcount = tight ? A.lookup_every_tight : A.lookup_every;
             const float ahead = tight ? 0.0f : A.lookahead;
             S.n = 0;
+            const float xh = lo(xyh), yh = hi(xyh), xl = lo(xyl), yl = hi(xyl), Txh = lo(Txyh), Tyh = hi(Txyh);
             const float cx = fmaf(ahead, Txh, xh), cy = fmaf(ahead, Tyh, yh), cz = fmaf(ahead, Tzh, zh);
             const float zeta = cz * A.gd.tan_abs;
             const float u2 = fmaf(cx, cx, fmaf(cy, cy, -zeta * zeta));
@@ -269,7 +293,8 @@ __global__ void __launch_bounds__(kBlock, FIELD == 0 ? 8 : 0) seed_scan_kernel(c
             }
         }
         kcount -= 1;
-        float sdx, sdy, sdz;                           // the increment this step adds to the position
+        f2 sdxy;                                       // the increment this step adds to the position
+        float sdz;
 
         // ---- A4: one Nystroem-RK4 step of r'' = a (r' x B(r))
         if (FIELD == 0) {
@@ -278,6 +303,7 @@ __global__ void __launch_bounds__(kBlock, FIELD == 0 ? 8 : 0) seed_scan_kernel(c
             //   dT = [ (theta - theta^3/6) J + (-theta^2/2 + theta^4/24) I ] T
             //   dr = h T + h [ (theta/2 - theta^3/24) J - (theta^2/6) I ] T          (k_z == 0, T_z constant)
             // -- the same map as k1..k4 and the weighted sums, with the stage arithmetic done once per seed.
+            // Packed: J T = (Ty, -Tx) is the pair with its halves swapped and one negated -- operand modifiers, no instruction.
             if (ELOSS) {                                  // theta follows p_n; constants in fp32 like a itself
                 const float th = a * A.fd.bz * h, th2 = th * th;
                 ub_h = fmaf(-th * th2, 0.166666672f, th); ub_l = ub_h * A.kq_rel;      // fl(kappa q) is off by the same
@@ -285,68 +311,66 @@ __global__ void __launch_bounds__(kBlock, FIELD == 0 ? 8 : 0) seed_scan_kernel(c
                 up1 = -h * th2 * 0.166666672f;
                 up2_h = h * th * fmaf(th2, -0.0416666679f, 0.5f); up2_l = up2_h * A.kq_rel;
             }
-            const float dTx = fmaf(ue1, Txh, fmaf(ub_h, Tyh, ub_l * Tyh));
-            const float dTy = fmaf(ue1, Tyh, -fmaf(ub_h, Txh, ub_l * Txh));
-            const float dx = fmaf(up1, Txh, fmaf(up2_h, Tyh, fmaf(up2_l, Tyh, h * Txh)));
-            const float dy = fmaf(up1, Tyh, -fmaf(up2_h, Txh, fmaf(up2_l, Txh, -h * Tyh)));
-            sdx = fmaf(h, Txl, dx); sdy = fmaf(h, Tyl, dy); sdz = fmaf(h, Tzl, h * Tzh);   // h * T_lo: the part of T
-            comp_add(xh, xl, sdx);                                                         // the fp32 products never saw
-            comp_add(yh, yl, sdy);
+            const f2 JT = pk(hi(Txyh), -lo(Txyh));     // J T: swap + negate one half, both operand modifiers (LO_HI.NP)
+            // dTx = fmaf(ue1, Tx, fmaf(ub_h, Ty, ub_l * Ty)),  dTy = fmaf(ue1, Ty, fmaf(ub_h, -Tx, ub_l * -Tx))
+            const f2 dTxy = fma2(bc(ue1), Txyh, fma2(bc(ub_h), JT, mul2(bc(ub_l), JT)));
+            // dx = fmaf(up1, Tx, fmaf(up2_h, Ty, fmaf(up2_l, Ty, h * Tx))),  dy likewise with -Tx for Ty and Ty for Tx
+            const f2 dxy = fma2(bc(up1), Txyh, fma2(bc(up2_h), JT, fma2(bc(up2_l), JT, mul2(h, Txyh))));
+            sdxy = fma2(bc(h), Txyl, dxy); sdz = fmaf(h, Tzl, h * Tzh);      // h * T_lo: the part of T the fp32 products
+            comp_add2(xyh, xyl, sdxy);                                       // never saw
             comp_add(zh, zl, sdz);
-            comp_add(Txh, Txl, dTx);
-            comp_add(Tyh, Tyl, dTy);
+            comp_add2(Txyh, Txyl, dTxy);
         } else {
-            float Bx, By, Bz;
-            field_at<FIELD>(A.fd, xh, yh, zh, Bx, By, Bz);
-            const float k1x = a * fmaf(Tyh, Bz, -Tzh * By), k1y = a * fmaf(Tzh, Bx, -Txh * Bz), k1z = a * fmaf(Txh, By, -Tyh * Bx);
-            float Ux = fmaf(A.h_half, k1x, Txh), Uy = fmaf(A.h_half, k1y, Tyh), Uz = fmaf(A.h_half, k1z, Tzh);
-            {
-                const float mx = fmaf(A.h2_8, k1x, fmaf(A.h_half, Txh, xh));
-                const float my = fmaf(A.h2_8, k1y, fmaf(A.h_half, Tyh, yh));
-                const float mz = fmaf(A.h2_8, k1z, fmaf(A.h_half, Tzh, zh));
-                field_at<FIELD>(A.fd, mx, my, mz, Bx, By, Bz);
-            }
-            const float k2x = a * fmaf(Uy, Bz, -Uz * By), k2y = a * fmaf(Uz, Bx, -Ux * Bz), k2z = a * fmaf(Ux, By, -Uy * Bx);
-            Ux = fmaf(A.h_half, k2x, Txh); Uy = fmaf(A.h_half, k2y, Tyh); Uz = fmaf(A.h_half, k2z, Tzh);
-            const float k3x = a * fmaf(Uy, Bz, -Uz * By), k3y = a * fmaf(Uz, Bx, -Ux * Bz), k3z = a * fmaf(Ux, By, -Uy * Bx);
-            Ux = fmaf(h, k3x, Txh); Uy = fmaf(h, k3y, Tyh); Uz = fmaf(h, k3z, Tzh);
-            {
-                const float ex = fmaf(A.h2_2, k3x, fmaf(h, Txh, xh));
-                const float ey = fmaf(A.h2_2, k3y, fmaf(h, Tyh, yh));
-                const float ez = fmaf(A.h2_2, k3z, fmaf(h, Tzh, zh));
-                field_at<FIELD>(A.fd, ex, ey, ez, Bx, By, Bz);
-            }
-            const float k4x = a * fmaf(Uy, Bz, -Uz * By), k4y = a * fmaf(Uz, Bx, -Ux * Bz), k4z = a * fmaf(Ux, By, -Uy * Bx);
-            const float dx = fmaf(A.h2_6, (k1x + k2x) + k3x, h * Txh);
-            const float dy = fmaf(A.h2_6, (k1y + k2y) + k3y, h * Tyh);
+            // stage derivatives k = a (U x B): the cross products mix components and stay scalar; their x and y results
+            // land side by side and everything linear in them (stage directions and positions, increments, compensated
+            // updates) is packed
+            f2 Bxy;
+            float Bz;
+            field_at_p(A.fd, xyh, zh, Bxy, Bz);
+            float Ux = lo(Txyh), Uy = hi(Txyh), Uz = Tzh;
+            const f2 k1xy = pk(a * fmaf(Uy, Bz, -Uz * hi(Bxy)), a * fmaf(Uz, lo(Bxy), -Ux * Bz));
+            const float k1z = a * fmaf(Ux, hi(Bxy), -Uy * lo(Bxy));
+            f2 Uxy = fma2(bc(A.h_half), k1xy, Txyh);
+            Uz = fmaf(A.h_half, k1z, Tzh);
+            field_at_p(A.fd, fma2(bc(A.h2_8), k1xy, fma2(bc(A.h_half), Txyh, xyh)), fmaf(A.h2_8, k1z, fmaf(A.h_half, Tzh, zh)), Bxy, Bz);
+            Ux = lo(Uxy); Uy = hi(Uxy);
+            const f2 k2xy = pk(a * fmaf(Uy, Bz, -Uz * hi(Bxy)), a * fmaf(Uz, lo(Bxy), -Ux * Bz));
+            const float k2z = a * fmaf(Ux, hi(Bxy), -Uy * lo(Bxy));
+            Uxy = fma2(bc(A.h_half), k2xy, Txyh); Uz = fmaf(A.h_half, k2z, Tzh);
+            Ux = lo(Uxy); Uy = hi(Uxy);
+            const f2 k3xy = pk(a * fmaf(Uy, Bz, -Uz * hi(Bxy)), a * fmaf(Uz, lo(Bxy), -Ux * Bz));
+            const float k3z = a * fmaf(Ux, hi(Bxy), -Uy * lo(Bxy));
+            Uxy = fma2(bc(h), k3xy, Txyh); Uz = fmaf(h, k3z, Tzh);
+            field_at_p(A.fd, fma2(bc(A.h2_2), k3xy, fma2(bc(h), Txyh, xyh)), fmaf(A.h2_2, k3z, fmaf(h, Tzh, zh)), Bxy, Bz);
+            Ux = lo(Uxy); Uy = hi(Uxy);
+            const f2 k4xy = pk(a * fmaf(Uy, Bz, -Uz * hi(Bxy)), a * fmaf(Uz, lo(Bxy), -Ux * Bz));
+            const float k4z = a * fmaf(Ux, hi(Bxy), -Uy * lo(Bxy));
+            const f2 dxy = fma2(bc(A.h2_6), add2(add2(k1xy, k2xy), k3xy), mul2(h, Txyh));
             const float dz = fmaf(A.h2_6, (k1z + k2z) + k3z, h * Tzh);
-            const float dTx = A.h_6 * fmaf(2.0f, k2x + k3x, k1x + k4x);
-            const float dTy = A.h_6 * fmaf(2.0f, k2y + k3y, k1y + k4y);
+            const f2 dTxy = mul2(A.h_6, fma2(bc(2.0f), add2(k2xy, k3xy), add2(k1xy, k4xy)));
             const float dTz = A.h_6 * fmaf(2.0f, k2z + k3z, k1z + k4z);
-            sdx = fmaf(h, Txl, dx); sdy = fmaf(h, Tyl, dy); sdz = fmaf(h, Tzl, dz);
-            comp_add(xh, xl, sdx);
-            comp_add(yh, yl, sdy);
+            sdxy = fma2(bc(h), Txyl, dxy); sdz = fmaf(h, Tzl, dz);
+            comp_add2(xyh, xyl, sdxy);
             comp_add(zh, zl, sdz);
-            comp_add(Txh, Txl, fmaf(dTx, epsT, dTx));
-            comp_add(Tyh, Tyl, fmaf(dTy, epsT, dTy));
+            comp_add2(Txyh, Txyl, fma2(dTxy, bc(epsT), dTxy));
             comp_add(Tzh, Tzl, fmaf(dTz, epsT, dTz));
         }
 
         // ---- A6: live wires over interval n (scored only if the interval starts in the gas)
         if (S.n > 0) {
             Vtx v1;
-            v1.x = xh; v1.xl = xl; v1.y = yh; v1.yl = yl; v1.z = zh;
+            v1.xy = xyh; v1.xyl = xyl; v1.z = zh;
             tests += (uint32_t)S.n;
-            slot_step(A, drift_e, S.w0, S.g0, cn, sdx, sdy, sdz, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
-            if (S.n > 1) slot_step(A, drift_e, S.w1, S.g1, cn, sdx, sdy, sdz, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
-            if (S.n > 2) slot_step(A, drift_e, S.w2, S.g2, cn, sdx, sdy, sdz, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
-            if (S.n > 3) slot_step(A, drift_e, S.w3, S.g3, cn, sdx, sdy, sdz, v1, Txh, Tyh, Tzh, nm, chi2, cnt);
+            slot_step(A, drift_e, S.w0, S.g0, cn, sdxy, sdz, v1, Txyh, Tzh, nm, chi2, cnt);
+            if (S.n > 1) slot_step(A, drift_e, S.w1, S.g1, cn, sdxy, sdz, v1, Txyh, Tzh, nm, chi2, cnt);
+            if (S.n > 2) slot_step(A, drift_e, S.w2, S.g2, cn, sdxy, sdz, v1, Txyh, Tzh, nm, chi2, cnt);
+            if (S.n > 3) slot_step(A, drift_e, S.w3, S.g3, cn, sdxy, sdz, v1, Txyh, Tzh, nm, chi2, cnt);
         }
         if (TRACK && cn) m += 1;
 
         // ---- advance, energy loss (reading C6), turn counter and termination (reading C7)
         n += 1;
-        float rho2 = fmaf(xh, xh, yh * yh);
+        float rho2 = fmaf(lo(xyh), lo(xyh), hi(xyh) * hi(xyh));
         if (TRACK) {
             bool cnext = rho2 >= A.gd.R0sq;
             if (!cn && cnext) turn += 1;
@@ -370,7 +394,7 @@ __global__ void __launch_bounds__(kBlock, FIELD == 0 ? 8 : 0) seed_scan_kernel(c
         if (A.debug) {
             cdc_seed_debug d;
             d.n_steps = n; d.turns = turn; d.m_gas = m; d.pad = 0;
-            d.x = (double)xh + (double)xl; d.y = (double)yh + (double)yl; d.z = (double)zh + (double)zl;
+            d.x = (double)lo(xyh) + (double)lo(xyl); d.y = (double)hi(xyh) + (double)hi(xyl); d.z = (double)zh + (double)zl;
             A.debug[o] = d;
         }
     }
@@ -432,6 +456,8 @@ cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0
     A.lambda = L.lambda; A.inv_lambda = 1.0f / L.lambda; A.eloss_h = L.eloss_h; A.window = sqrtf(L.lambda) * 1.0001f;
     A.u2_lo = L.u2_lo; A.u2_hi = L.u2_hi; A.uz = L.uz; A.inv_uz = L.inv_uz; A.lookup_every = L.lookup_every; A.lookahead = L.lookahead; A.lookup_every_tight = L.lookup_every_tight; A.tight_curv = L.tight_curv;
     A.delta_max = L.delta_max; A.b_max = L.b_max; A.hold_path = L.hold_path;
+    A.k_margin = L.k_margin; A.k_margin0 = L.k_margin0; A.sin_eps = L.sin_eps; A.sep_cap = L.sep_cap;
+    A.two_inv_h = (float)(2.0 / h); A.inv_h = (float)(1.0 / h);
     A.max_steps = L.max_steps; A.margin = L.margin;
     A.n_match = L.d_n_match; A.chi2 = L.d_chi2; A.debug = L.d_debug;
     A.best_key = (unsigned long long *)L.d_best_key;
@@ -443,8 +469,16 @@ cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0
     // a held wire is scored from vertices at most `back` inside the lookup band's lower edge: if that is still outside
     // R0 the in-gas flag is true whenever it is read (c_0 := true covers the start vertex)
     const double u_lo = sqrt((double)L.u2_lo);
-    const double back = std::max((double)L.lookahead + 0.2, (L.lookup_every_tight - 1) * h);
+    const double back = (double)L.back;
     const bool track = eloss || L.d_debug != nullptr || !(u_lo - back - 0.5 >= sqrt((double)L.gd.R0sq));
+    // comparison variant (params.kernel_variant = 1): two seeds per thread (scan_pair.cu); it has no tabulated-field
+    // form with energy loss (per-seed momentum), which stays with the kernel below
+    if (L.variant == 1 && !(L.fd.kind != 0 && eloss)) {
+        const cudaError_t pe = launch_seed_scan_pair(A, L, eloss, track, s);
+        if (k1) cudaEventRecord(k1, s);
+        cdc_count_launch();
+        return pe;
+    }
     if (L.fd.kind == 0) {
         if (eloss) seed_scan_kernel<0, true, true><<<grid, kBlock, 0, s>>>(A);
         else if (track) seed_scan_kernel<0, false, true><<<grid, kBlock, 0, s>>>(A);

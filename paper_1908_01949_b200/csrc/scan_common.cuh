@@ -38,6 +38,9 @@ __device__ __forceinline__ float coarse_atan2(float y, float x)
     return copysignf(p, y);
 }
 
+constexpr float kMagicRound = 12582912.0f;          // 1.5 * 2^23
+constexpr int kMagicRoundBits = 0x4B400000;
+
 template <int FIELD>
 __device__ __forceinline__ void field_at(const FieldDev &F, float x, float y, float z, float &Bx, float &By,
                                          float &Bz)
@@ -45,19 +48,23 @@ __device__ __forceinline__ void field_at(const FieldDev &F, float x, float y, fl
     if (FIELD == 0) {
         Bx = 0.0f; By = 0.0f; Bz = F.bz;
     } else {
-        // validated at create time: the table covers every point a live track or its stages can reach, so the
-        // cell index needs no lower clamp; the unsigned min only keeps a non-finite state inside the allocation
+        // validated at create time: the table covers every point a live track or its stages can reach; the unsigned
+        // min on the cell number only keeps a non-finite state inside the allocation.
+        // Nearest cell centre by the magic-number rounding (adding 1.5 * 2^23 leaves the rounded integer in the low
+        // mantissa bits): no F2I / I2F, and in the two-seed kernel one packed add serves both seeds.  The per-cell
+        // coefficients are taken about the cell centre, so the offsets wr, wz lie in [-1/2, 1/2].
         const float rho2 = fmaf(x, x, y * y);
         const float inv_rho = rsqrt_normal(fmaxf(rho2, 1e-30f));
         const float rho = rho2 * inv_rho;
-        const float fr = fmaf(rho, F.inv_dr, F.cr), fz = fmaf(z, F.inv_dz, F.cz);
-        const unsigned ir = min((unsigned)__float2int_rd(fr), (unsigned)(F.nr - 2));
-        const unsigned iz = min((unsigned)__float2int_rd(fz), (unsigned)(F.nz - 2));
-        const float wr = fr - (float)ir, wz = fz - (float)iz;
-        const float4 *c = F.cells + 2u * (iz * (unsigned)(F.nr - 1) + ir);
-        const float4 cr = __ldg(c), cz = __ldg(c + 1);
-        const float Br = fmaf(wz, fmaf(wr, cr.w, cr.z), fmaf(wr, cr.y, cr.x));
-        Bz = fmaf(wz, fmaf(wr, cz.w, cz.z), fmaf(wr, cz.y, cz.x));
+        const float fr = fmaf(rho, F.inv_dr, F.cr), fz = fmaf(z, F.inv_dz, F.cz);     // cell coordinate - 1/2
+        const float tr = fr + kMagicRound, tz = fz + kMagicRound;
+        const float wr = fr - (tr - kMagicRound), wz = fz - (tz - kMagicRound);
+        const int ir = __float_as_int(tr) - kMagicRoundBits, iz = __float_as_int(tz) - kMagicRoundBits;
+        const unsigned cell = min((unsigned)(iz * (F.nr - 1) + ir), (unsigned)(F.n_cells - 1));
+        const float4 *c = F.cells + 2u * cell;
+        const float4 cr = __ldg(c), cz = __ldg(c + 1);                   // (c0, c_z, c_r, c_rz) of B_r, of B_z
+        const float Br = fmaf(wz, fmaf(wr, cr.w, cr.y), fmaf(wr, cr.z, cr.x));
+        Bz = fmaf(wz, fmaf(wr, cz.w, cz.y), fmaf(wr, cz.z, cz.x));
         const float s = Br * inv_rho;
         Bx = s * x; By = s * y;
     }
