@@ -173,8 +173,11 @@ int32_t cdc_scan_get_stats(const cdc_events *ev, cdc_scan_stats *h_out, void *st
  * in IEEE fp64 without FMA contraction; the maximum of S (ties: lowest index) is the best seed; its matched
  * approaches label each hit with a turn index, or -1.  Per event: d_best_seed i64, d_best_n_match u32,
  * d_best_chi2 f64; d_labels i32 per hit (events concatenated in upload order).  Must follow cdc_seed_scan on
- * the same stream with the same grids / params.  Asynchronous; pool overflow is reported by the next
- * cdc_scan_get_stats (n_pool > pool_cap) and by cdc_find_tracks_host. */
+ * the same stream with the same grids / params.  Synchronises `stream` once (an 8-byte read-back of the number of
+ * candidates, which sizes the launches).  The candidate pool cannot silently lose the best seed: if the scan appended
+ * more candidates than the pool holds (many near-ties, e.g. a plateau of identical seeds), the near-ties of the FINAL
+ * fp32 maximum are collected again by a second pass of the scan into a pool sized for them (up to 2^26 entries;
+ * beyond that CDC_ERR_RANGE).  cdc_scan_get_stats().n_pool is then the second pass's count. */
 int32_t cdc_best_track(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec *h_grids,
                        const cdc_scan_params *params, const uint64_t *d_best_key, int64_t *d_best_seed,
                        uint32_t *d_best_n_match, double *d_best_chi2, int32_t *d_labels, void *stream);

@@ -86,7 +86,6 @@ extern "C" int32_t cdc_find_tracks_host(const cdc_geometry *g, int32_t n_events,
     cdc_scan_stats st;
     rc = cdc_scan_get_stats(S.ev, &st, stream);           // synchronises
     if (rc != CDC_OK) return rc;
-    if (st.n_pool > st.pool_cap) CDC_FAIL(CDC_ERR_RANGE, "cdc_find_tracks_host: candidate pool overflow");
     return CDC_OK;
     });
 }

@@ -13,7 +13,11 @@ void free_events(cdc_events *ev)
 {
     if (!ev) return;
     // stream-ordered: the memory returns to the pool after the work already queued on the upload stream
+    // work queued on another stream (scan / best track are asynchronous on a caller-chosen stream) must have finished
+    // before the memory goes back to the pool
+    if (ev->last_stream && ev->last_stream != ev->alloc_stream) cudaStreamSynchronize(ev->last_stream);
     if (ev->slab) cudaFreeAsync(ev->slab, ev->alloc_stream);
+    if (ev->big_slab) cudaFreeAsync(ev->big_slab, ev->alloc_stream);
     if (ev->axes.d) cudaFreeAsync(ev->axes.d, ev->alloc_stream);
     if (ev->ev_k0) cudaEventDestroy(ev->ev_k0);
     if (ev->ev_k1) cudaEventDestroy(ev->ev_k1);

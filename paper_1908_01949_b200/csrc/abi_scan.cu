@@ -113,6 +113,81 @@ int32_t prepare_grids(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec
     return CDC_OK;
 }
 
+// everything of a scan launch that follows from the geometry, the scanned grids and the parameters (the per-call
+// output pointers are set by the caller)
+int32_t fill_scan_launch(const cdc_geometry *g, const cdc_events *ev, const cdc_scan_params *p, ScanLaunch &L)
+{
+    L.gd = g->gd; L.fd = g->fd; L.n_events = ev->n_events; L.d_grids = ev->d_grids; L.d_axes = ev->axes.d;
+    L.axis_stride = ev->axes.stride; L.d_drift_tab = ev->d_drift_tab; L.d_bits = ev->d_bits;
+    L.h = (float)p->h_mm; L.h64 = p->h_mm; L.lambda = (float)(p->window_mm * p->window_mm);
+    L.eloss_h = (float)(p->eloss_MeV_per_mm * p->h_mm);
+    L.max_steps = p->max_steps; L.charge = p->charge;
+    L.margin = (float)(p->rescore_margin > 0.0 ? p->rescore_margin : kDefaultMargin);
+    L.d_n_match = nullptr; L.d_chi2 = nullptr; L.d_debug = nullptr; L.d_best_key = nullptr;
+    L.d_pool = ev->d_pool; L.pool_cap = ev->pool_cap; L.d_counters = ev->d_counters;
+    // lookup cadence K: the 2 x 2 candidate set is taken around c = r_n + (K h / 2) T_n, the middle of the next K steps.
+    // A wire that can own a match in interval n + i lies within `reach` of vertex n + i, which lies within K h / 2 (+ the
+    // sagitta of that arc) of c; every wire outside the set is at least `excl` away from c (reading C8).
+    {
+        const double dmax = 8.0 + p->window_mm + 0.05;           // largest matching D: drift <= 8 mm (upload check)
+        const double reach = sqrt(dmax * dmax + p->h_mm * p->h_mm) + 0.1;
+        if (reach > g->excl) CDC_FAIL(CDC_ERR_RANGE, "cdc_seed_scan: window + step too large for the 2 x 2 wire lookup");
+        const double sag = 0.15;                                 // (K h / 2)^2 / (2 R) for R >= 150 mm, K h / 2 <= 6.7 mm
+        int K = (int)floor(2.0 * (g->excl - reach - sag) / p->h_mm);
+        K = std::max(1, std::min(K, 16));
+        double ahead = 0.5 * K * p->h_mm;
+        if (ahead + reach + sag > g->excl) { K = 1; ahead = 0.0; }
+        L.lookup_every = K; L.lookahead = (float)ahead;
+        // the straight-line prediction of the centre needs a track radius well above K h (the kernel checks
+        // |a| B_max < 1 / 20 mm per seed); tighter curls look up around r_n itself, every K0 steps
+        const int K0 = std::max(1, std::min(1 + (int)floor((g->excl - reach) / p->h_mm), 16));
+        L.lookup_every_tight = K0;
+        // vertex n + i lies i h along the arc: (i h - ahead) along the tangent from c and at most kappa (i h)^2 / 2 off
+        // it, so it stays within ahead + sag of c for every i <= K iff kappa <= 2 sqrt(sag^2 + 2 sag ahead) / (K h)^2
+        // (kappa = |a| B_max, the track's curvature bound); never above the old fixed 1 / 20 mm
+        {
+            const double Kh = K * p->h_mm;
+            L.tight_curv = (float)(ahead > 0.0 ? std::min(0.05, 0.98 * 2.0 * sqrt(sag * sag + 2.0 * sag * ahead) / (Kh * Kh)) : 0.05);
+        }
+        // the two-seed kernel looks wires up around the midpoint of its two seeds, at most sep_cap (as a wire sees it)
+        // from either seed's own centre: every bound that speaks of "the lookup centre" is widened by it
+        const bool pair = p->kernel_variant == 1 && !(g->field.kind != 0 && p->eloss_MeV_per_mm > 0.0);
+        const double sep_cap = pair ? 1.5 : 0.0;
+        L.sep_cap = (float)sep_cap;
+        L.k_margin = (float)(0.9999 * (g->excl - reach - sag) - 0.01);
+        L.k_margin0 = (float)(0.9999 * (g->excl - reach) - 0.01);
+        {
+            double se = 0.0;
+            for (int j = 0; j < g->n_layers; ++j) se = std::max(se, fabs(sin(g->stereo[j])));
+            L.sin_eps = (float)(1.0001 * se);
+        }
+        const double grow = reach + 0.2 + sep_cap + std::max(ahead + sag, (K0 - 1) * p->h_mm);
+        const double ulo = std::max(g->r[0] - grow, 0.0), uhi = g->r[g->n_layers - 1] + grow;
+        L.u2_lo = (float)(ulo * ulo); L.u2_hi = (float)(uhi * uhi);
+        L.back = (float)(std::max(ahead + 0.2, (K0 - 1) * p->h_mm) + sep_cap);
+        L.uz = g->uz; L.inv_uz = (float)(1.0 / (double)g->uz);
+        // a held wire lies within the 2 x 2 set of the last lookup vertex (two layer pitches x two cells) and
+        // the track has moved at most K h since: |delta| <= diag + K h; it stays held while the track crosses
+        // that neighbourhood, at most ~(diag + K h) / min|T_perp| of path -- bounded here by 4 diag
+        const double diag = hypot(2.0 * g->pitch, 2.0 * g->cell_max);
+        // the kernel's curvature bounds allow |a| = kappa / p to grow by 5 % between two lookups; p > 1 MeV/c on a live
+        // track, so the momentum lost over one lookup period must stay below 0.04 MeV/c
+        if (p->eloss_MeV_per_mm * (std::max(K, K0) * p->h_mm + 1.0) > 0.04)
+            CDC_FAIL(CDC_ERR_RANGE, "cdc_seed_scan: energy loss too large for the lookup cadence (eloss * K h must stay below 0.04 MeV/c)");
+        L.delta_max = (float)(diag + std::max(K, K0) * p->h_mm + 1.0 + sep_cap);
+        L.b_max = (float)(1.001 * g->b_max);
+        L.hold_path = (float)(4.0 * diag + 2.0 * std::max(K, K0) * p->h_mm + 2.0 * sep_cap);
+    }
+    L.max_seeds_per_event = 0;
+    L.max_pairs_per_event = 0;
+    for (const GridDev &G : ev->h_grids) {
+        L.max_seeds_per_event = std::max<int64_t>(L.max_seeds_per_event, G.n_seeds);
+        L.max_pairs_per_event = std::max<int64_t>(L.max_pairs_per_event, ((int64_t)G.n_seeds / G.n[1]) * ((G.n[1] + 1) / 2));
+    }
+    L.variant = p->kernel_variant;
+    return CDC_OK;
+}
+
 }  // namespace
 
 int32_t cdc_lookup_every64(const cdc_geometry *g, double h_mm, double window_mm)
@@ -179,77 +254,12 @@ extern "C" int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cd
     CDC_CUDA(cudaMemsetAsync(d_best_key, 0, sizeof(uint64_t) * (size_t)ev->n_events, s));
     CDC_CUDA(cudaMemsetAsync(ev->d_counters, 0, sizeof(unsigned long long) * CNT_N, s));
     ScanLaunch L;
-    L.gd = g->gd; L.fd = g->fd; L.n_events = ev->n_events; L.d_grids = ev->d_grids; L.d_axes = ev->axes.d;
-    L.axis_stride = ev->axes.stride; L.d_drift_tab = ev->d_drift_tab; L.d_bits = ev->d_bits;
-    L.h = (float)p->h_mm; L.h64 = p->h_mm; L.lambda = (float)(p->window_mm * p->window_mm);
-    L.eloss_h = (float)(p->eloss_MeV_per_mm * p->h_mm);
-    L.max_steps = p->max_steps; L.charge = p->charge;
-    L.margin = (float)(p->rescore_margin > 0.0 ? p->rescore_margin : kDefaultMargin);
+    if ((rc = fill_scan_launch(g, ev, p, L)) != CDC_OK) return rc;
     L.d_n_match = d_n_match; L.d_chi2 = d_chi2; L.d_debug = d_debug; L.d_best_key = d_best_key;
-    L.d_pool = ev->d_pool; L.pool_cap = ev->pool_cap; L.d_counters = ev->d_counters;
-    // lookup cadence K: the 2 x 2 candidate set is taken around c = r_n + (K h / 2) T_n, the middle of the next K steps.
-    // A wire that can own a match in interval n + i lies within `reach` of vertex n + i, which lies within K h / 2 (+ the
-    // sagitta of that arc) of c; every wire outside the set is at least `excl` away from c (reading C8).
-    {
-        const double dmax = 8.0 + p->window_mm + 0.05;           // largest matching D: drift <= 8 mm (upload check)
-        const double reach = sqrt(dmax * dmax + p->h_mm * p->h_mm) + 0.1;
-        if (reach > g->excl) CDC_FAIL(CDC_ERR_RANGE, "cdc_seed_scan: window + step too large for the 2 x 2 wire lookup");
-        const double sag = 0.15;                                 // (K h / 2)^2 / (2 R) for R >= 150 mm, K h / 2 <= 6.7 mm
-        int K = (int)floor(2.0 * (g->excl - reach - sag) / p->h_mm);
-        K = std::max(1, std::min(K, 16));
-        double ahead = 0.5 * K * p->h_mm;
-        if (ahead + reach + sag > g->excl) { K = 1; ahead = 0.0; }
-        L.lookup_every = K; L.lookahead = (float)ahead;
-        // the straight-line prediction of the centre needs a track radius well above K h (the kernel checks
-        // |a| B_max < 1 / 20 mm per seed); tighter curls look up around r_n itself, every K0 steps
-        const int K0 = std::max(1, std::min(1 + (int)floor((g->excl - reach) / p->h_mm), 16));
-        L.lookup_every_tight = K0;
-        // vertex n + i lies i h along the arc: (i h - ahead) along the tangent from c and at most kappa (i h)^2 / 2 off
-        // it, so it stays within ahead + sag of c for every i <= K iff kappa <= 2 sqrt(sag^2 + 2 sag ahead) / (K h)^2
-        // (kappa = |a| B_max, the track's curvature bound); never above the old fixed 1 / 20 mm
-        {
-            const double Kh = K * p->h_mm;
-            L.tight_curv = (float)(ahead > 0.0 ? std::min(0.05, 0.98 * 2.0 * sqrt(sag * sag + 2.0 * sag * ahead) / (Kh * Kh)) : 0.05);
-        }
-        // the two-seed kernel looks wires up around the midpoint of its two seeds, at most sep_cap (as a wire sees it)
-        // from either seed's own centre: every bound that speaks of "the lookup centre" is widened by it
-        const bool pair = p->kernel_variant == 1 && !(g->field.kind != 0 && p->eloss_MeV_per_mm > 0.0);
-        const double sep_cap = pair ? 1.5 : 0.0;
-        L.sep_cap = (float)sep_cap;
-        L.k_margin = (float)(0.9999 * (g->excl - reach - sag) - 0.01);
-        L.k_margin0 = (float)(0.9999 * (g->excl - reach) - 0.01);
-        {
-            double se = 0.0;
-            for (int j = 0; j < g->n_layers; ++j) se = std::max(se, fabs(sin(g->stereo[j])));
-            L.sin_eps = (float)(1.0001 * se);
-        }
-        const double grow = reach + 0.2 + sep_cap + std::max(ahead + sag, (K0 - 1) * p->h_mm);
-        const double ulo = std::max(g->r[0] - grow, 0.0), uhi = g->r[g->n_layers - 1] + grow;
-        L.u2_lo = (float)(ulo * ulo); L.u2_hi = (float)(uhi * uhi);
-        L.back = (float)(std::max(ahead + 0.2, (K0 - 1) * p->h_mm) + sep_cap);
-        L.uz = g->uz; L.inv_uz = (float)(1.0 / (double)g->uz);
-        // a held wire lies within the 2 x 2 set of the last lookup vertex (two layer pitches x two cells) and
-        // the track has moved at most K h since: |delta| <= diag + K h; it stays held while the track crosses
-        // that neighbourhood, at most ~(diag + K h) / min|T_perp| of path -- bounded here by 4 diag
-        const double diag = hypot(2.0 * g->pitch, 2.0 * g->cell_max);
-        // the kernel's curvature bounds allow |a| = kappa / p to grow by 5 % between two lookups; p > 1 MeV/c on a live
-        // track, so the momentum lost over one lookup period must stay below 0.04 MeV/c
-        if (p->eloss_MeV_per_mm * (std::max(K, K0) * p->h_mm + 1.0) > 0.04)
-            CDC_FAIL(CDC_ERR_RANGE, "cdc_seed_scan: energy loss too large for the lookup cadence (eloss * K h must stay below 0.04 MeV/c)");
-        L.delta_max = (float)(diag + std::max(K, K0) * p->h_mm + 1.0 + sep_cap);
-        L.b_max = (float)(1.001 * g->b_max);
-        L.hold_path = (float)(4.0 * diag + 2.0 * std::max(K, K0) * p->h_mm + 2.0 * sep_cap);
-    }
-    L.max_seeds_per_event = 0;
-    L.max_pairs_per_event = 0;
-    for (const GridDev &G : ev->h_grids) {
-        L.max_seeds_per_event = std::max<int64_t>(L.max_seeds_per_event, G.n_seeds);
-        L.max_pairs_per_event = std::max<int64_t>(L.max_pairs_per_event, ((int64_t)G.n_seeds / G.n[1]) * ((G.n[1] + 1) / 2));
-    }
-    L.variant = p->kernel_variant;
     if (!ev->ev_k0) { CDC_CUDA(cudaEventCreate(&ev->ev_k0)); CDC_CUDA(cudaEventCreate(&ev->ev_k1)); }
     CDC_CUDA(launch_seed_scan(L, s, ev->ev_k0, ev->ev_k1));
     ev->scanned = true;
+    ev->last_stream = s;
     return CDC_OK;
     });
 }
@@ -290,6 +300,54 @@ extern "C" int32_t cdc_best_track(const cdc_geometry *g, cdc_events *ev, const c
     for (int e = 0; e < ev->n_events; ++e)
         for (int a = 0; a < 5; ++a)
             if (h_grids[e].n[a] != ev->h_grids[e].n[a]) CDC_FAIL(CDC_ERR_INVALID, "cdc_best_track: grids differ from the scanned ones");
+    cudaStream_t s = (cudaStream_t)stream;
+    ev->last_stream = s;
+    // how many candidates did the scan append?  (one 8-byte read-back; the launches below are sized by it)
+    unsigned long long n_pool = 0;
+    CDC_CUDA(cudaMemcpyAsync(&n_pool, ev->d_counters + CNT_POOL, sizeof(n_pool), cudaMemcpyDeviceToHost, s));
+    CDC_CUDA(cudaStreamSynchronize(s));
+    PoolEntry *pool = ev->d_pool;
+    double *pS64 = ev->d_pool_S64, *pchi2 = ev->d_pool_chi2;
+    int32_t *pnm = ev->d_pool_nmatch, *pslot = ev->d_pool_slot;
+    uint32_t cap = ev->pool_cap;
+    if (n_pool > (unsigned long long)ev->pool_cap) {
+        // Overflow: the pool was filled against the RUNNING maximum, in launch order, so what it holds is arbitrary.
+        // Collect again against the FINAL maximum: the scan is repeated with best_key left as it is (every seed now sees
+        // the final maximum as the running one) and a pool as large as the first pass's count, an upper bound of what
+        // the second can append (the final threshold is the highest).  Bounded by the true number of near-ties.
+        if (n_pool > (1ull << 26))
+            CDC_FAIL(CDC_ERR_RANGE, "cdc_best_track: more than 2^26 seeds within the re-score margin of the running maximum");
+        if ((unsigned long long)ev->big_cap < n_pool) {
+            if (ev->big_slab) CDC_CUDA(cudaFreeAsync(ev->big_slab, s));
+            ev->big_slab = nullptr; ev->big_cap = 0;
+            const size_t n = (size_t)n_pool, a = 256;
+            const size_t o1 = (n * sizeof(PoolEntry) + a - 1) / a * a, o2 = o1 + (n * 8 + a - 1) / a * a, o3 = o2 + (n * 8 + a - 1) / a * a,
+                         o4 = o3 + (n * 4 + a - 1) / a * a, o5 = o4 + (n * 4 + a - 1) / a * a;
+            CDC_CUDA(cudaMallocAsync(&ev->big_slab, o5, s));
+            char *b = static_cast<char *>(ev->big_slab);
+            ev->d_bpool = reinterpret_cast<PoolEntry *>(b); ev->d_bS64 = reinterpret_cast<double *>(b + o1);
+            ev->d_bchi2 = reinterpret_cast<double *>(b + o2); ev->d_bnmatch = reinterpret_cast<int32_t *>(b + o3);
+            ev->d_bslot = reinterpret_cast<int32_t *>(b + o4);
+            ev->big_cap = (uint32_t)n_pool;
+        }
+        unsigned long long saved[CNT_N];
+        CDC_CUDA(cudaMemcpyAsync(saved, ev->d_counters, sizeof(saved), cudaMemcpyDeviceToHost, s));
+        CDC_CUDA(cudaStreamSynchronize(s));
+        CDC_CUDA(cudaMemsetAsync(ev->d_counters + CNT_POOL, 0, sizeof(unsigned long long), s));
+        ScanLaunch SL;
+        if ((rc = fill_scan_launch(g, ev, p, SL)) != CDC_OK) return rc;
+        SL.d_best_key = const_cast<uint64_t *>(d_best_key);          // atomicMax with values that cannot exceed it: unchanged
+        SL.d_pool = ev->d_bpool; SL.pool_cap = ev->big_cap;
+        CDC_CUDA(launch_seed_scan(SL, s, nullptr, nullptr));
+        CDC_CUDA(cudaMemcpyAsync(&n_pool, ev->d_counters + CNT_POOL, sizeof(n_pool), cudaMemcpyDeviceToHost, s));
+        CDC_CUDA(cudaStreamSynchronize(s));
+        saved[CNT_POOL] = n_pool;                                     // the scan's work counters stay those of the first pass
+        CDC_CUDA(cudaMemcpyAsync(ev->d_counters, saved, sizeof(saved), cudaMemcpyHostToDevice, s));
+        CDC_CUDA(cudaStreamSynchronize(s));
+        if (n_pool > (unsigned long long)ev->big_cap) CDC_FAIL(CDC_ERR_RANGE, "cdc_best_track: candidate pool overflow in the second pass");
+        pool = ev->d_bpool; pS64 = ev->d_bS64; pchi2 = ev->d_bchi2; pnm = ev->d_bnmatch; pslot = ev->d_bslot; cap = ev->big_cap;
+    }
+    ev->last_pool_count = n_pool;
     BestLaunch L;
     L.g = g->g64; L.n_events = ev->n_events; L.d_grids = ev->d_grids; L.d_axes = ev->axes.d; L.axis_stride = ev->axes.stride;
     L.d_offsets = ev->d_offsets; L.d_wire_id = ev->d_wire_id; L.d_drift = ev->d_drift; L.d_drift_tab = ev->d_drift_tab;
@@ -297,10 +355,10 @@ extern "C" int32_t cdc_best_track(const cdc_geometry *g, cdc_events *ev, const c
     L.h = p->h_mm; L.window = p->window_mm; L.eloss = p->eloss_MeV_per_mm; L.max_steps = p->max_steps; L.charge = p->charge;
     L.lookup_every64 = cdc_lookup_every64(g, p->h_mm, p->window_mm);
     L.margin = (float)(p->rescore_margin > 0.0 ? p->rescore_margin : kDefaultMargin);
-    L.d_best_key = d_best_key; L.d_pool = ev->d_pool; L.pool_cap = ev->pool_cap; L.d_counters = ev->d_counters;
-    L.d_pool_S64 = ev->d_pool_S64; L.d_pool_chi2 = ev->d_pool_chi2; L.d_pool_nmatch = ev->d_pool_nmatch;
+    L.d_best_key = d_best_key; L.d_pool = pool; L.pool_cap = cap; L.n_entries = (uint32_t)n_pool; L.d_counters = ev->d_counters;
+    L.d_pool_S64 = pS64; L.d_pool_chi2 = pchi2; L.d_pool_nmatch = pnm;
     L.d_ev_maxS = ev->d_ev_maxS; L.d_ev_best = ev->d_ev_best; L.d_wire_label = ev->d_wire_label; L.d_wire_best = ev->d_wire_best;
-    L.d_rec = ev->d_rec; L.d_rec_count = ev->d_rec_count; L.d_pool_slot = ev->d_pool_slot; L.d_slot_counter = ev->d_slot_counter;
+    L.d_rec = ev->d_rec; L.d_rec_count = ev->d_rec_count; L.d_pool_slot = pslot; L.d_slot_counter = ev->d_slot_counter;
     L.d_ev_slot = ev->d_ev_slot;
     L.d_best_seed = d_best_seed; L.d_best_n_match = d_best_n_match; L.d_best_chi2 = d_best_chi2; L.d_labels = d_labels;
     CDC_CUDA(launch_best_track(L, (cudaStream_t)stream));

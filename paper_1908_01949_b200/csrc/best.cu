@@ -10,6 +10,8 @@
 //   PAPER.md:55,:69  DCA, left/right ambiguity                 -> eval_seed64()
 //   PAPER.md:65-69   Eq. (1), S = n_match - chi2 / lambda      -> rescore_kernel / pick_kernel
 //   PAPER.md:69      "hits with d^2 < lambda are classified"   -> label_kernel
+#include <algorithm>
+
 #include "cdc_internal.cuh"
 
 #include "eval64.cuh"
@@ -156,8 +158,10 @@ cudaError_t launch_best_track(const BestLaunch &L, cudaStream_t s)
     if ((e = cudaMemsetAsync(L.d_ev_best, 0xFF, sizeof(unsigned long long) * (size_t)L.n_events, s)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(L.d_ev_slot, 0xFF, sizeof(int32_t) * (size_t)L.n_events, s)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(L.d_slot_counter, 0, sizeof(int32_t), s)) != cudaSuccess) return e;
-    const unsigned nb = (L.pool_cap + 63) / 64;
-    rescore_kernel<<<(L.pool_cap + 3) / 4, 128, 0, s>>>(A, L.d_pool, L.pool_cap, L.d_counters, L.d_best_key, L.margin, L.d_pool_S64,
+    // grids sized by the number of entries the pool actually holds (read back by cdc_best_track), not by its capacity
+    const unsigned ne = std::max(1u, std::min(L.n_entries, L.pool_cap));
+    const unsigned nb = (ne + 63) / 64;
+    rescore_kernel<<<(ne + 3) / 4, 128, 0, s>>>(A, L.d_pool, L.pool_cap, L.d_counters, L.d_best_key, L.margin, L.d_pool_S64,
                                      L.d_pool_chi2, L.d_pool_nmatch, L.d_ev_maxS, L.d_rec, L.d_rec_count, L.d_pool_slot,
                                      L.d_slot_counter);
     pick_kernel<<<nb, 64, 0, s>>>(L.d_pool, L.pool_cap, L.d_counters, L.d_pool_S64, L.d_ev_maxS, L.d_ev_best);

@@ -143,6 +143,15 @@ struct cdc_events {
     int32_t *d_pool_slot = nullptr;             // [pool_cap] record slot of a pool entry, -1 = none
     int32_t *d_slot_counter = nullptr;
     int32_t *d_ev_slot = nullptr;               // per event: record slot of the best seed, -1 = re-propagate
+    // overflow pool (cdc_best_track): when the scan appended more candidates than pool_cap, the near-ties of the FINAL
+    // maximum are collected again into a pool sized for them
+    void *big_slab = nullptr;
+    uint32_t big_cap = 0;
+    PoolEntry *d_bpool = nullptr;
+    double *d_bS64 = nullptr, *d_bchi2 = nullptr;
+    int32_t *d_bnmatch = nullptr, *d_bslot = nullptr;
+    unsigned long long last_pool_count = 0;     // entries the last cdc_best_track re-scored from (after any second pass)
+    cudaStream_t last_stream = nullptr;         // stream of the last asynchronous call on this batch
     // one stream-ordered allocation holds every device buffer above
     void *slab = nullptr;
     cudaStream_t alloc_stream = nullptr;
@@ -247,6 +256,7 @@ struct BestLaunch {
     const uint64_t *d_best_key;
     const PoolEntry *d_pool;
     uint32_t pool_cap;
+    uint32_t n_entries;                      // pool entries to re-score (host copy of the counter, <= pool_cap)
     const unsigned long long *d_counters;
     double *d_pool_S64, *d_pool_chi2;
     int32_t *d_pool_nmatch;

@@ -336,3 +336,38 @@ def test_every_wire_fired_at_the_corners_of_step_and_window(field_kind, h, windo
     assert bad.size <= int(5e-3 * grid.n_seeds)
     U.check_best(cfg, geom, field, ev, grid, gpu, orc_full=orc)
     sc.close()
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_candidate_pool_overflow_is_recovered_by_a_second_pass(setup, variant):
+    """More near-ties than the candidate pool holds: a plateau grid -- step = 0 on four
+    axes, 16^5 = 1,048,576 nodes of which only 16 are distinct, each 65,536 times -- fills the 65,536-entry pool in
+    launch order, against the running maximum.  cdc_best_track must collect the near-ties of the FINAL maximum again
+    (second pass of the scan into a pool sized for them) and return the exact best seed: the LOWEST linear index among
+    the copies of the best node (reading C10), its n_match / chi2 bit-equal to the oracle's, and the labels."""
+    cfg, geom, field, events, grids, sc = setup
+    ev = events[0]
+    full, _ = synth.truth_anchored_grid(ev.seed, 16)
+    lo = ev.seed.copy(); lo[4] = full.lo[4]
+    step = np.zeros(5); step[4] = full.step[4]
+    grid = synth.Grid(lo=lo, step=step, n=np.full(5, 16, dtype=np.int32))
+    off, w, d = synth.pack_hits([ev])
+    E = sc.upload(off, w, d)
+    gpu = sc.scan(E, [grid], U.gpu_params(cfg, kernel_variant=variant), per_seed=False, debug=False)
+    st = gpu["stats"]
+    assert st["pool_cap"] == 65536 and st["n_pool"] >= 65536          # the second pass's count: every copy of the best node
+    line = synth.Grid(lo=lo, step=step, n=np.array([1, 1, 1, 1, 16], dtype=np.int32))
+    bound = oracle.Bound(geom, field, U.oracle_params(cfg))
+    o = oracle.scan(bound, ev.wire_id, ev.drift_mm, line)
+    k, _ = oracle.argmax(o["n_match"], o["chi2"], cfg.window_mm)
+    assert int(gpu["best_seed"][0]) == k                               # theta, z, px, py indices 0: linear index = i_pz
+    assert int(gpu["best_n_match"][0]) == int(o["n_match"][k]) and float(gpu["best_chi2"][0]) == float(o["chi2"][k])
+    lab, _ = oracle.labels(bound, ev.wire_id, ev.drift_mm, line.node((0, 0, 0, 0, k)))
+    assert np.array_equal(gpu["labels"], lab)
+    # an ordinary scan on the same handle afterwards is unaffected
+    g2 = grids[0]
+    again = sc.scan(E, [g2], U.gpu_params(cfg, kernel_variant=variant), per_seed=False, debug=False)
+    E2 = sc.upload(off, w, d)
+    fresh = sc.scan(E2, [g2], U.gpu_params(cfg, kernel_variant=variant), per_seed=False, debug=False)
+    for key in ("best_seed", "best_n_match", "best_chi2", "labels", "best_key"):
+        assert np.array_equal(again[key], fresh[key]), key
