@@ -182,16 +182,17 @@ int32_t cdc_best_track(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spe
                        const cdc_scan_params *params, const uint64_t *d_best_key, int64_t *d_best_seed,
                        uint32_t *d_best_n_match, double *d_best_chi2, int32_t *d_labels, void *stream);
 
-/* The whole path with host buffers in and out (upload, optional Hough ranges, scan, best track, read-back):
- * the end-to-end call.  If hp is non-NULL the (theta, px, py) axes of every grid are replaced by n[a] nodes
- * spanning the Hough ranges (BJ configs[2]); h_zref_mm is then required.  Outputs (host): h_best_seed,
- * h_best_n_match, h_best_chi2, h_best_key per event; h_labels per hit; h_ranges_or_null [n_events][3][2].
- * Synchronises. */
+/* The whole path with host buffers in and out (upload, optional Hough vote, scan, best track, read-back): the
+ * end-to-end call.  If hp is non-NULL the Hough vote runs (h_zref_mm required) and its ranges are returned in
+ * h_ranges_or_null [n_events][3][2]; if hough_sets_axes is also non-zero the (theta, px, py) axes of every grid are
+ * replaced by n[a] nodes spanning those ranges (BJ configs[2]: "Hough pre-vote narrows the ranges"), otherwise the grids
+ * are scanned as given.  Outputs (host): h_best_seed, h_best_n_match, h_best_chi2, h_best_key per event; h_labels per
+ * hit.  Synchronises. */
 int32_t cdc_find_tracks_host(const cdc_geometry *g, int32_t n_events, const int32_t *h_hit_offsets,
                              const int32_t *h_wire_id, const float *h_drift_mm, const cdc_grid_spec *h_grids,
                              const cdc_scan_params *params, const cdc_hough_params *hp_or_null,
-                             const float *h_zref_mm_or_null, int64_t *h_best_seed, uint32_t *h_best_n_match,
-                             double *h_best_chi2, uint64_t *h_best_key, int32_t *h_labels,
+                             const float *h_zref_mm_or_null, int32_t hough_sets_axes, int64_t *h_best_seed,
+                             uint32_t *h_best_n_match, double *h_best_chi2, uint64_t *h_best_key, int32_t *h_labels,
                              double *h_ranges_or_null, void *stream);
 
 /* Coarse-to-fine refinement around the seed scan ("we took the several candidate seeds with the lowest

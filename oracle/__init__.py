@@ -72,6 +72,21 @@ def lib():
     return _lib
 
 
+def timed_with_fast_build(fn):
+    """Run fn() with the speed build of the same source loaded (bench.py's second CPU number), then restore the
+    parity build.  Timing only."""
+    global _lib
+    lib()
+    keep = _lib
+    fast = C.CDLL(_build.build_fast())
+    fast.orc_argmax.restype = C.c_int64
+    try:
+        _lib = fast
+        return fn()
+    finally:
+        _lib = keep
+
+
 def _p(a: Optional[np.ndarray]):
     return None if a is None else a.ctypes.data_as(C.c_void_p)
 

@@ -79,9 +79,9 @@ class SeedScanner:
         return out
 
     def find_tracks_host(self, hit_offsets, wire_id, drift_mm, grids: Sequence, params: B.ScanParams,
-                         hp: Optional[B.HoughParams] = None, zref=None) -> dict:
+                         hp: Optional[B.HoughParams] = None, zref=None, hough_sets_axes: bool = True) -> dict:
         return B.cdc_find_tracks_host(self.geometry, hit_offsets, wire_id, drift_mm, B.grid_specs(grids), params,
-                                      hp, zref)
+                                      hp, zref, hough_sets_axes)
 
     def refine(self, events: B.Events, grids: Sequence, params: B.ScanParams, n_parents: int = 8,
                n_iterations: int = 10, **kw) -> dict:

@@ -245,8 +245,9 @@ def cdc_best_track(geometry: Geometry, events: Events, grids: C.Array, params: S
 
 
 def cdc_find_tracks_host(geometry: Geometry, hit_offsets, wire_id, drift_mm, grids: C.Array, params: ScanParams,
-                         hp: Optional[HoughParams] = None, zref=None, stream=None) -> dict:
-    """End-to-end call with host (numpy) buffers in and out."""
+                         hp: Optional[HoughParams] = None, zref=None, hough_sets_axes: bool = True, stream=None) -> dict:
+    """End-to-end call with host (numpy) buffers in and out.  With hp the Hough vote runs; its ranges replace the
+    (theta, px, py) axes of the grids unless hough_sets_axes is False."""
     off = np.ascontiguousarray(hit_offsets, dtype=np.int32)
     w = np.ascontiguousarray(wire_id, dtype=np.int32); d = np.ascontiguousarray(drift_mm, dtype=np.float32)
     E = int(off.size - 1)
@@ -255,7 +256,8 @@ def cdc_find_tracks_host(geometry: Geometry, hit_offsets, wire_id, drift_mm, gri
     ranges = np.zeros((E, 3, 2)) if hp is not None else None
     zr = None if zref is None else np.ascontiguousarray(zref, dtype=np.float32)
     _check(lib().cdc_find_tracks_host(geometry.handle, C.c_int32(E), _hp(off), _hp(w), _hp(d), grids, C.byref(params),
-                                      None if hp is None else C.byref(hp), _hp(zr), _hp(seed), _hp(nm), _hp(chi2),
+                                      None if hp is None else C.byref(hp), _hp(zr), C.c_int32(1 if hough_sets_axes else 0),
+                                      _hp(seed), _hp(nm), _hp(chi2),
                                       _hp(key), _hp(lab), _hp(ranges), _stream(stream)))
     return dict(best_seed=seed, best_n_match=nm, best_chi2=chi2, best_key=key, labels=lab[:int(off[-1])],
                 ranges=ranges)

@@ -33,7 +33,7 @@ struct Scratch {                       // device buffers of one call, freed on e
 extern "C" int32_t cdc_find_tracks_host(const cdc_geometry *g, int32_t n_events, const int32_t *h_hit_offsets,
                                         const int32_t *h_wire_id, const float *h_drift_mm, const cdc_grid_spec *h_grids,
                                         const cdc_scan_params *params, const cdc_hough_params *hp,
-                                        const float *h_zref_mm, int64_t *h_best_seed, uint32_t *h_best_n_match,
+                                        const float *h_zref_mm, int32_t hough_sets_axes, int64_t *h_best_seed, uint32_t *h_best_n_match,
                                         double *h_best_chi2, uint64_t *h_best_key, int32_t *h_labels,
                                         double *h_ranges, void *stream)
 {
@@ -64,7 +64,7 @@ extern "C" int32_t cdc_find_tracks_host(const cdc_geometry *g, int32_t n_events,
         CDC_CUDA(cudaMemcpyAsync(rg.data(), S.ranges, sizeof(double) * 6 * E, cudaMemcpyDeviceToHost, s));
         CDC_CUDA(cudaStreamSynchronize(s));
         const int axis_of[3] = {0, 2, 3};                 // Hough gives theta, px, py
-        for (size_t e = 0; e < E; ++e)
+        for (size_t e = 0; hough_sets_axes && e < E; ++e)
             for (int k = 0; k < 3; ++k) {
                 const int a = axis_of[k];
                 const double lo = rg[6 * e + 2 * k], hi = rg[6 * e + 2 * k + 1];

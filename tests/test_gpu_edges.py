@@ -194,6 +194,13 @@ def test_host_call_with_hough_ranges(setup):
     for k in ("best_seed", "best_n_match", "best_chi2", "labels"):
         assert np.array_equal(out[k], staged[k]), k
     U.check_best(cfg2, geom, field, ev, grid, staged)
+    # the vote without the replacement of the axes (bench.py's end-to-end arm on truth-anchored grids): same ranges
+    # reported, the grid scanned as given
+    keep = sc.find_tracks_host(off, w, d, [g0], P, hp=B.hough_params(), zref=[float(ev.seed[1])], hough_sets_axes=False)
+    plain = sc.scan(E, [g0], P, per_seed=False)
+    assert np.array_equal(keep["ranges"], h["ranges"])
+    for k in ("best_seed", "best_n_match", "best_chi2", "labels", "best_key"):
+        assert np.array_equal(keep[k], plain[k]), k
 
 
 def test_fp32_peak_probe_is_near_nominal():
