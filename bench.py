@@ -59,33 +59,13 @@ def parse():
     return ap.parse_args()
 
 
-def _gen_chunk(job):
-    cfg_id, first, n = job
-    cfg = synth.CONFIGS[cfg_id]
-    geom = synth.make_geometry()
-    field = synth.make_uniform_field() if cfg.field_kind == 0 else synth.make_table_field()
-    return synth.generate_events(cfg, geom, field, n, first_event=first)
-
-
-def generate_events_parallel(cfg_id, n_events, first_event):
-    """The seeded generator, event ranges spread over the host cores (an event depends on its index only)."""
-    chunk = 8
-    jobs = [(cfg_id, first_event + i, min(chunk, n_events - i)) for i in range(0, n_events, chunk)]
-    if len(jobs) == 1:
-        return _gen_chunk(jobs[0])
-    import multiprocessing as mp
-    with mp.get_context("fork").Pool(min(len(jobs), os.cpu_count() or 1)) as pool:
-        parts = pool.map(_gen_chunk, jobs)
-    return [e for p in parts for e in p]
-
-
 def make_workload(args, rank, workload=None):
     cfg_id = int((workload or args.workload)[3:])
     cfg = synth.CONFIGS[cfg_id]
     geom = synth.make_geometry()
     field = synth.make_uniform_field() if cfg.field_kind == 0 else synth.make_table_field()
     n_events = (args.events if workload is None else 0) or cfg.n_events
-    events = generate_events_parallel(cfg_id, n_events, rank * n_events)
+    events = synth.generate_events_parallel(cfg_id, n_events, rank * n_events)
     n = (args.grid_n if workload is None else 0) or cfg.grid_n
     grids = [synth.truth_anchored_grid(ev.seed, n)[0] for ev in events]
     return cfg_id, cfg, geom, field, events, grids

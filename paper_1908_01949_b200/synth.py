@@ -472,6 +472,27 @@ def generate_events(cfg: EventConfig, geom: Geometry, field: Field, n_events: Op
     return done  # type: ignore[return-value]
 
 
+def _generate_chunk(job):
+    cfg_id, first, n, kw = job
+    cfg = CONFIGS[cfg_id]
+    geom = make_geometry()
+    field = make_uniform_field() if cfg.field_kind == 0 else make_table_field()
+    return generate_events(cfg, geom, field, n, first_event=first, **kw)
+
+
+def generate_events_parallel(cfg_id: int, n_events: int, first_event: int = 0, chunk: int = 8, **kw) -> List["Event"]:
+    """generate_events() for the default geometry / field of config cfg_id with the event ranges spread over the host
+    cores (an event depends on its index only, so the result is the same list)."""
+    import multiprocessing as mp
+    import os
+    jobs = [(cfg_id, first_event + i, min(chunk, n_events - i), kw) for i in range(0, n_events, chunk)]
+    if len(jobs) <= 1:
+        return _generate_chunk(jobs[0]) if jobs else []
+    with mp.get_context("fork").Pool(min(len(jobs), os.cpu_count() or 1)) as pool:
+        parts = pool.map(_generate_chunk, jobs)
+    return [e for p in parts for e in p]
+
+
 # --------------------------------------------------------------------------
 # seed grids
 # --------------------------------------------------------------------------
