@@ -45,6 +45,10 @@ def parse():
     ap.add_argument("--kernel-variant", type=int, default=0, choices=[0, 1],
                     help="0 = production scan kernel, 1 = the two-seeds-per-thread comparison variant")
     ap.add_argument("--no-secondary", action="store_true", help="skip the short configs[1] measurement")
+    ap.add_argument("--shard", default="auto", choices=["auto", "events", "theta"],
+                    help="with N GPUs: 'events' = every rank scans its own events (weak scaling, no collective); 'theta' = "
+                         "all ranks scan the SAME events, each a slab of the theta axis, exact winners merged by one "
+                         "all_gather + one all_reduce (strong scaling); auto = events if the workload has >= N events")
     ap.add_argument("--grid-n", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true",
@@ -182,7 +186,11 @@ def measure(args, workload, steps, warmup, rank, world, local, dist, with_cpu_ba
     """One workload through the whole hot path: device-timed arm, end-to-end arm, roofline of the scan kernel."""
     import torch
     from paper_1908_01949_b200 import api, binding as B
-    cfg_id, cfg, geom, field, events, grids = make_workload(args, rank, None if workload == args.workload else workload)
+    cfg0 = synth.CONFIGS[int(workload[3:])]
+    n_ev = (args.events if workload == args.workload else 0) or cfg0.n_events
+    theta = args.shard == "theta" or (args.shard == "auto" and world > 1 and n_ev < world)
+    cfg_id, cfg, geom, field, events, grids = make_workload(args, 0 if theta else rank,
+                                                            None if workload == args.workload else workload)
     sc = api.SeedScanner(geom, field)
     off, w, d = synth.pack_hits(events)
     E = len(events)
@@ -199,7 +207,11 @@ def measure(args, workload, steps, warmup, rank, world, local, dist, with_cpu_ba
             lo = g.lo.copy(); hi = g.lo + g.step * (g.n - 1)
             lo[[0, 2, 3]] = rg[e][:, 0]; hi[[0, 2, 3]] = rg[e][:, 1]
             grids[e] = synth.ranges_grid(lo, hi, g.n)
-    n_seeds = sum(g.n_seeds for g in grids)
+    full_grids = grids
+    slab_off = None
+    if theta:                                          # this rank's slab of every grid (node values bit-identical to the full grid's)
+        grids, slab_off = sc.slabs(full_grids, rank, world)
+    n_seeds = sum(g.n_seeds for g, o in zip(grids, slab_off or [0] * len(grids)) if o >= 0)
     specs = B.grid_specs(grids)
     # device-resident inputs and outputs of the device-timed arm
     d_w = torch.tensor(w, device="cuda"); d_d = torch.tensor(d, device="cuda"); d_zref = torch.tensor(zref, device="cuda")
@@ -215,7 +227,15 @@ def measure(args, workload, steps, warmup, rank, world, local, dist, with_cpu_ba
         B.cdc_hough_seed_ranges(sc.geometry, ev, hp, -1, d_zref, d_ranges, d_peak)  # A2
         B.cdc_seed_scan(sc.geometry, ev, specs, P, d_key)                           # A3-A7
         B.cdc_best_track(sc.geometry, ev, specs, P, d_key, d_seed, d_nm, d_c2, d_lab)   # A8-A9
+        if theta:                                      # exact winners of the slabs -> the event's best seed and labels
+            from paper_1908_01949_b200 import dist as D
+            torch.cuda.synchronize()
+            res = dict(best_seed=d_seed.cpu().numpy(), best_n_match=d_nm.cpu().numpy().astype(np.uint32),
+                       best_chi2=d_c2.cpu().numpy(), labels=d_lab.cpu().numpy()[:int(off[-1])])
+            merged[0] = D.merge_slab_results_collective(res, slab_off, cfg.window_mm, off, device=torch.device("cuda", local))
         return ev
+
+    merged = [None]
 
     def barrier():
         if world > 1:
@@ -244,6 +264,8 @@ def measure(args, workload, steps, warmup, rank, world, local, dist, with_cpu_ba
     launches = B.cdc_kernel_launch_count() - l0
     clocks = sampler.stop()
     best = (d_seed.cpu().numpy().tolist(), d_nm.cpu().numpy().tolist())
+    if theta:
+        best = (merged[0]["best_seed"].tolist(), merged[0]["best_n_match"].tolist())
 
     # end to end: host buffers through the C ABI (cdc_find_tracks_host: A1, A2, A3-A9), H2D + D2H inside the timed
     # region, wall clock around the call.  The same steps as the device-timed arm: the Hough vote runs; its ranges
@@ -254,6 +276,8 @@ def measure(args, workload, steps, warmup, rank, world, local, dist, with_cpu_ba
     if cfg.hough_axes:
         e2e_grids = [synth.truth_anchored_grid(evn.seed, g.n)[0] for evn, g in zip(events, grids)]   # (z, pz) axes; the rest is replaced
     e2e_steps = max(1, min(steps, 5)) if E >= 64 else steps
+    if theta:
+        e2e_grids = full_grids                         # the end-to-end call is the one-GPU call: every rank runs the whole event
     sc.find_tracks_host(h_off, h_w, h_d, e2e_grids, P, hp=hp, zref=zref, hough_sets_axes=bool(cfg.hough_axes))
     barrier()
     t0 = time.perf_counter()
@@ -272,6 +296,11 @@ def measure(args, workload, steps, warmup, rank, world, local, dist, with_cpu_ba
         dist.all_reduce(t, op=dist.ReduceOp.MAX); dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
     total_ms, e2e_s, ksum_ms = t.tolist()
     seeds_all, steps_all, events_all = cnt.tolist()
+    if theta:
+        events_all = float(E)                          # the same events on every rank
+        e2e_seeds = float(sum(g.n_seeds for g in full_grids))
+    else:
+        e2e_seeds = seeds_all
     if rank != 0:
         return None
     K = steps
@@ -282,7 +311,7 @@ def measure(args, workload, steps, warmup, rank, world, local, dist, with_cpu_ba
     traffic, traffic_source = measured_traffic(workload)
     line = {"metric": METRIC, "value": seeds_all * K / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
             "warmup": warmup, "ms_per_step": total_ms / K, "ms_per_step_median": float(np.median(ms)),
-            "ms_per_step_max": float(np.max(ms)), "higher_is_better": True, "scaling": "weak",
+            "ms_per_step_max": float(np.max(ms)), "higher_is_better": True, "scaling": "strong" if theta else "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload, "events_per_gpu": E, "seeds_per_event": grids[0].n_seeds,
                        "max_steps": cfg.max_steps, "h_mm": cfg.h_mm, "field": "table" if cfg.field_kind else "uniform",
@@ -290,13 +319,15 @@ def measure(args, workload, steps, warmup, rank, world, local, dist, with_cpu_ba
                        "seed_axes": "theta, px, py from the Hough ranges; z, pz truth-anchored" if cfg.hough_axes
                        else "truth-anchored (the Hough vote runs, its ranges are not used for the grid)",
                        "kernel_variant": args.kernel_variant,
-                       "parallelism": f"dp{world} (events sharded over ranks, no data-path collective)"},
+                       "parallelism": (f"theta{world} (every rank scans a theta slab of the same events; exact winners merged "
+                                       f"by one all_gather + one all_reduce(MAX), a few bytes per event)") if theta
+                       else f"dp{world} (events sharded over ranks, no data-path collective)"},
             "rkn_steps_per_s": steps_all * 1.0 / (total_ms * 1e-3), "events_per_s": events_all * K / (total_ms * 1e-3),
             "scan_kernel_ms": sum(kernel_ms) / K, "scan_kernel_share": ksum_ms / total_ms,
             "rkn_steps_per_s_kernel": acc["n_steps"] / k_s,
             "candidate_pool": {"entries_per_step": acc["n_pool"] / K, "capacity": int(st["pool_cap"])},
             "clocks": clocks,
-            "e2e": {"value": seeds_all / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+            "e2e": {"value": e2e_seeds / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps, "call": "cdc_find_tracks_host (A1, A2 Hough vote, A3-A9)"},
             "gpu_launches": int(launches),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_FP32_TFLOPS, "unit": "TFLOP/s",

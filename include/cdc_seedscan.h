@@ -67,10 +67,14 @@ typedef struct {
     const float *h_br_bz;
 } cdc_field_desc;
 
-/* 5-D seed grid of one event: axis a (theta, z, px, py, pz) has n[a] nodes lo[a] + i step[a]. */
+/* 5-D seed grid of one event: axis a (theta, z, px, py, pz) has n[a] nodes lo[a] + (first[a] + i) step[a], i = 0 ..
+ * n[a] - 1.  first[a] (>= 0, normally 0) lets a slab of a larger grid be scanned with node values that are
+ * bit-identical to the larger grid's (one event split over several GPUs along theta); the linear
+ * seed index is local to the slab.  cdc_refine_tracks and cdc_peel_turns require first = 0. */
 typedef struct {
     double lo[5], step[5];
     int32_t n[5];
+    int32_t first[5];
 } cdc_grid_spec;
 
 /* Propagation and scoring parameters (BJ configs[0]: fixed 2 mm step, <= 1500 steps, 1 mm window).

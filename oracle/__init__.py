@@ -251,3 +251,65 @@ def bin_event(bound: Bound, wire_id, drift) -> np.ndarray:
     out = np.zeros(bound.n_wires_total, dtype=np.float32)
     lib().orc_bin_event(C.byref(bound.g), C.byref(H), _p(out))
     return out
+
+
+class OrcAdaptiveInfo(C.Structure):
+    _fields_ = [("units", C.c_int32), ("n_level", C.c_int32 * 8), ("margin_tol", C.c_double), ("margin_up", C.c_double)]
+
+
+def eval_seed_adaptive(bound: Bound, wire_id, drift, seed, tol: float, h_max: float, records: bool = False,
+                       rec_slack: float = 0.0):
+    """One seed with the adaptive step of reading C19 applied to the scan (orc_eval_seed_adaptive).  Returns the fields
+    of eval_seed plus units (path in units of h), n_level (accepted steps per level) and the decision margins."""
+    H, _ = bound.hits(wire_id, drift)
+    seed = np.ascontiguousarray(seed, dtype=np.float64)
+    res = OrcResult(); info = OrcAdaptiveInfo()
+    cap = (64 * max(int(H.n_hits), 1) + 4096) if records else 0
+    rec = np.zeros(cap, dtype=APPROACH_DTYPE) if records else None
+    lib().orc_eval_seed_adaptive(C.byref(bound.g), C.byref(bound.f), C.byref(H), _p(seed), C.byref(bound.P),
+                                 C.c_double(tol), C.c_double(h_max), C.byref(res), C.byref(info), _p(rec), C.c_int32(cap),
+                                 C.c_double(rec_slack))
+    out = dict(n_match=res.n_match, chi2=res.chi2, n_steps=res.n_steps, turns=res.turns, m_gas=res.m_gas,
+               r=np.array(res.r[:]), T=np.array(res.T[:]), p=res.p, units=info.units, n_level=np.array(info.n_level[:]),
+               margin_tol=info.margin_tol, margin_up=info.margin_up)
+    if records:
+        out["rec"] = rec[:res.n_rec]
+    return out
+
+
+def scan_adaptive(bound: Bound, wire_id, drift, grid, tol: float, h_max: float, index_list=None, begin: int = 0,
+                  end: Optional[int] = None):
+    H, _ = bound.hits(wire_id, drift)
+    lo = np.ascontiguousarray(grid.lo, dtype=np.float64); st = np.ascontiguousarray(grid.step, dtype=np.float64)
+    nn = np.ascontiguousarray(grid.n, dtype=np.int32)
+    il = None if index_list is None else np.ascontiguousarray(index_list, dtype=np.int64)
+    if end is None:
+        end = int(il.size) if il is not None else int(np.prod(nn.astype(np.int64)))
+    n = end - begin
+    nm = np.zeros(n, dtype=np.int32); c2 = np.zeros(n); ns = np.zeros(n, dtype=np.int32); un = np.zeros(n, dtype=np.int32)
+    mg = np.zeros(n, dtype=np.int32); fr = np.zeros((n, 3)); nl = np.zeros((n, 8), dtype=np.int32); mar = np.zeros((n, 2))
+    lib().orc_scan_adaptive(C.byref(bound.g), C.byref(bound.f), C.byref(H), _p(lo), _p(st), _p(nn), _p(il),
+                            C.c_int64(begin), C.c_int64(end), C.byref(bound.P), C.c_double(tol), C.c_double(h_max),
+                            _p(nm), _p(c2), _p(ns), _p(un), _p(mg), _p(fr), _p(nl), _p(mar))
+    return dict(n_match=nm, chi2=c2, n_steps=ns, units=un, m_gas=mg, final_r=fr, n_level=nl, margins=mar)
+
+
+def _scan_adaptive_worker(args):
+    geom, field, params, wire_id, drift, grid, tol, h_max, il, b, e = args
+    return scan_adaptive(Bound(geom, field, params), wire_id, drift, grid, tol, h_max, il, b, e)
+
+
+def scan_adaptive_parallel(geom, field, params: dict, wire_id, drift, grid, tol: float, h_max: float, index_list=None,
+                           n_proc: Optional[int] = None):
+    import multiprocessing as mp
+    total = int(index_list.size) if index_list is not None else grid.n_seeds
+    n_proc = n_proc or min(os.cpu_count() or 1, 8)
+    edges = np.linspace(0, total, max(1, min(total, n_proc * 4)) + 1).astype(np.int64)
+    jobs = [(geom, field, params, wire_id, drift, grid, tol, h_max, index_list, int(edges[i]), int(edges[i + 1]))
+            for i in range(len(edges) - 1) if edges[i + 1] > edges[i]]
+    if n_proc == 1 or len(jobs) == 1:
+        parts = [_scan_adaptive_worker(j) for j in jobs]
+    else:
+        with mp.get_context("fork").Pool(n_proc) as pool:
+            parts = pool.map(_scan_adaptive_worker, jobs)
+    return {k: np.concatenate([p[k] for p in parts]) for k in parts[0]}

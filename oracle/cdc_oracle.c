@@ -313,6 +313,128 @@ void orc_eval_seed(const orc_geom *g, const orc_field *f, const orc_hits *hits,
     out->p = p; out->n_rec = n_rec;
 }
 
+void orc_seed_of_index(const double *lo, const double *step, const int32_t *nn, int64_t idx, double *seed);
+
+/* ---- The same evaluation with the ADAPTIVE step of the propagator the paper cites ("the RKN method was
+ * used for the track parameter propagation [5]"; [5] = Lund et al.) -- reading C19 applied to the scan
+ * (SURVEY 8(f) #4).  Step lengths are h 2^j, j = 0..J with h 2^J <= h_max.  A trial step of length h 2^j has the error
+ * estimate err = (h 2^j)^2 max_i |k1 - k2 - k3 + k4|_i (orc_rkn_step_err); if err > tol and j > 0 the trial is repeated
+ * with j - 1; otherwise it is accepted, and after an accepted step with err <= tol / 32 the next trial starts one level
+ * up (the estimate grows ~16-fold per doubling).  Path is counted in units of h: the step cap max_steps is a PATH cap
+ * (a trial that would exceed it drops to the level that fits), the in-gas count m sums the units of the steps that
+ * start in the gas, and p = p0 - eps h m (reading C6 generalised).  Everything else -- ownership of an approach by the
+ * sign change of g over the (now longer) interval, chord interpolation, window, turn counter, termination -- is C7-C10
+ * unchanged; the candidate wires are ALL hit wires (mode 0: the plain definition).
+ * Outputs beyond orc_result: units (path in units of h), n_level[j] accepted steps per level (j < 8), and the decision
+ * margins min |err - tol| / tol over rejections / acceptances and min |err - tol/32| / (tol/32) over the doubling
+ * decisions (a GPU that takes its decisions in fp32 can differ where these are ~ 1e-5). */
+typedef struct {
+    int32_t units, n_level[8];
+    double margin_tol, margin_up;
+} orc_adaptive_info;
+
+void orc_eval_seed_adaptive(const orc_geom *g, const orc_field *f, const orc_hits *hits, const double *seed,
+                            const orc_params *P, double tol, double h_max, orc_result *out, orc_adaptive_info *info,
+                            orc_approach *rec, int32_t rec_cap, double rec_slack)
+{
+    double r[3], T[3], rn[3], Tn[3];
+    double lambda = P->window * P->window;
+    double p0, p, err;
+    int32_t n = 0, t = 0, m = 0, n_match = 0, n_rec = 0, units = 0, j = 0, J = 0, ic;
+    double chi2 = 0.0;
+    int c_n = 1, c_next, i;
+    while (J < 7 && P->h * (double)(2 << J) <= h_max) ++J;      /* h 2^(J+1) <= h_max -> J + 1 */
+    for (i = 0; i < 8; ++i) info->n_level[i] = 0;
+    info->margin_tol = 1e300; info->margin_up = 1e300;
+    r[0] = g->R0 * cos(seed[0]); r[1] = g->R0 * sin(seed[0]); r[2] = seed[1];
+    p0 = sqrt(seed[2] * seed[2] + seed[3] * seed[3] + seed[4] * seed[4]);
+    T[0] = seed[2] / p0; T[1] = seed[3] / p0; T[2] = seed[4] / p0;
+    p = p0;
+    while (units < P->max_steps) {
+        double a = (ORC_KAPPA * (double)P->charge) / p;
+        double hj, mt;
+        while (j > 0 && units + (1 << j) > P->max_steps) --j;          /* the path cap */
+        for (;;) {
+            hj = P->h * (double)(1 << j);
+            orc_rkn_step_err(f, a, hj, r, T, rn, Tn, &err);
+            mt = fabs(err - tol) / tol;
+            if (mt < info->margin_tol) info->margin_tol = mt;
+            if (err > tol && j > 0) { --j; continue; }
+            break;
+        }
+        if (c_n) {
+            for (ic = 0; ic < hits->n_hits; ++ic) {
+                const float *w = g->wire + (size_t)hits->wire_id[ic] * 5;
+                double g0 = wire_g(w, r, T), g1, tau, Pp[3], d[3], tpar, D, zw, x, resid;
+                int inside, matched;
+                if (!(g0 <= 0.0)) continue;
+                g1 = wire_g(w, rn, Tn);
+                if (!(g1 > 0.0)) continue;
+                tau = g0 / (g0 - g1);
+                for (i = 0; i < 3; ++i) Pp[i] = r[i] + tau * (rn[i] - r[i]);
+                wire_delta(w, Pp, d, &tpar);
+                D = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+                zw = tpar * (double)w[4];
+                x = (double)hits->drift[ic];
+                resid = D - x;
+                inside = fabs(zw) <= g->z_half;
+                matched = inside && (resid * resid < lambda);
+                if (matched) { n_match += 1; chi2 += resid * resid; }
+                if (rec && n_rec < rec_cap && D < x + P->window + rec_slack) {
+                    orc_approach *q = rec + n_rec++;
+                    q->interval = n; q->hit = ic; q->wire = hits->wire_id[ic]; q->turn = t; q->matched = matched;
+                    q->D = D; q->resid = resid; q->zw = zw;
+                }
+            }
+            m += 1 << j;
+        }
+        for (i = 0; i < 3; ++i) { r[i] = rn[i]; T[i] = Tn[i]; }
+        n += 1; units += 1 << j; info->n_level[j] += 1;
+        p = p0 - (P->eloss * P->h) * (double)m;
+        c_next = (r[0] * r[0] + r[1] * r[1] >= g->R0 * g->R0);
+        if (!c_n && c_next) t += 1;
+        c_n = c_next;
+        if (fabs(r[2]) > g->z_half) break;
+        if (r[0] * r[0] + r[1] * r[1] > g->r_out * g->r_out) break;
+        if (!(p > 1.0)) break;
+        if (!(isfinite(r[0]) && isfinite(r[1]) && isfinite(r[2]) &&
+              isfinite(T[0]) && isfinite(T[1]) && isfinite(T[2]))) break;
+        if (j < J) {
+            double mu = fabs(err - tol / 32.0) / (tol / 32.0);
+            if (mu < info->margin_up) info->margin_up = mu;
+            if (err <= tol / 32.0) ++j;
+        }
+    }
+    out->n_match = n_match; out->chi2 = chi2; out->n_steps = n; out->turns = t; out->m_gas = m;
+    for (i = 0; i < 3; ++i) { out->r[i] = r[i]; out->T[i] = T[i]; }
+    out->p = p; out->n_rec = n_rec;
+    info->units = units;
+}
+
+/* exhaustive adaptive-step evaluation of a list of seeds (or of seeds [begin, end) of the grid) */
+void orc_scan_adaptive(const orc_geom *g, const orc_field *f, const orc_hits *hits,
+                       const double *lo, const double *step, const int32_t *nn, const int64_t *index_list,
+                       int64_t begin, int64_t end, const orc_params *P, double tol, double h_max,
+                       int32_t *n_match, double *chi2, int32_t *n_steps, int32_t *units, int32_t *m_gas, double *final_r,
+                       int32_t *n_level /* [..][8] */, double *margins /* [..][2] */)
+{
+    int64_t s;
+    int i;
+    for (s = begin; s < end; ++s) {
+        double seed[5];
+        orc_result res;
+        orc_adaptive_info info;
+        int64_t idx = index_list ? index_list[s] : s;
+        int64_t o = s - begin;
+        orc_seed_of_index(lo, step, nn, idx, seed);
+        orc_eval_seed_adaptive(g, f, hits, seed, P, tol, h_max, &res, &info, NULL, 0, 0.0);
+        n_match[o] = res.n_match; chi2[o] = res.chi2; n_steps[o] = res.n_steps; units[o] = info.units; m_gas[o] = res.m_gas;
+        final_r[3 * o] = res.r[0]; final_r[3 * o + 1] = res.r[1]; final_r[3 * o + 2] = res.r[2];
+        for (i = 0; i < 8; ++i) n_level[8 * o + i] = info.n_level[i];
+        margins[2 * o] = info.margin_tol; margins[2 * o + 1] = info.margin_up;
+    }
+}
+
 /* seed linear index -> 5 values; axes theta, z, px, py, pz; pz fastest (tie-break order) */
 void orc_seed_of_index(const double *lo, const double *step, const int32_t *nn, int64_t idx, double *seed)
 {

@@ -78,6 +78,37 @@ class SeedScanner:
             out["debug"] = d_dbg.cpu().numpy().view(B.SEED_DEBUG_DTYPE)
         return out
 
+    def slabs(self, grids: Sequence, rank: int, world: int):
+        """This rank's theta slab of every grid (dist.shard_theta) and the index offsets back to the full grids; an
+        event whose theta axis has fewer nodes than ranks gets a one-node placeholder here and offset -1 (ignored)."""
+        import copy
+        from . import dist as D
+        subs, offs = [], []
+        for g in grids:
+            sub, off = D.shard_theta(g, rank, world)
+            if sub is None:
+                sub = copy.deepcopy(g)
+                sub.n = np.ones(5, dtype=np.int32); sub.first = np.zeros(5, dtype=np.int32)
+                off = -1
+            subs.append(sub); offs.append(off)
+        return subs, offs
+
+    def scan_sharded(self, events: B.Events, grids: Sequence, params: B.ScanParams, rank: int, world: int,
+                     hit_offsets, collective: bool = True) -> dict:
+        """One event batch whose seed grids are split over `world` GPUs along theta: this rank
+        scans its slabs (node values bit-identical to the full grids'), re-scores its near-best seeds exactly, and the
+        ranks' exact winners are merged (highest fp64 S, then lowest global index).  collective=True merges over
+        torch.distributed and returns the merged result on every rank; collective=False returns this rank's own
+        (result, offsets) for dist.merge_slab_results."""
+        from . import dist as D
+        subs, offs = self.slabs(grids, rank, world)
+        res = self.scan(events, subs, params, per_seed=False, debug=False)
+        if not collective:
+            return dict(result=res, offsets=offs)
+        torch = _torch()
+        return D.merge_slab_results_collective(res, offs, float(params.window_mm), np.asarray(hit_offsets),
+                                               device=torch.device("cuda", torch.cuda.current_device()))
+
     def find_tracks_host(self, hit_offsets, wire_id, drift_mm, grids: Sequence, params: B.ScanParams,
                          hp: Optional[B.HoughParams] = None, zref=None, hough_sets_axes: bool = True) -> dict:
         return B.cdc_find_tracks_host(self.geometry, hit_offsets, wire_id, drift_mm, B.grid_specs(grids), params,

@@ -40,7 +40,7 @@ class FieldDesc(C.Structure):
 
 
 class GridSpec(C.Structure):
-    _fields_ = [("lo", C.c_double * 5), ("step", C.c_double * 5), ("n", C.c_int32 * 5)]
+    _fields_ = [("lo", C.c_double * 5), ("step", C.c_double * 5), ("n", C.c_int32 * 5), ("first", C.c_int32 * 5)]
 
 
 class ScanParams(C.Structure):
@@ -129,11 +129,13 @@ def hough_params(**kw) -> HoughParams:
 
 
 def grid_specs(grids: Sequence) -> C.Array:
-    """Objects with .lo, .step, .n (5 each) -> array of cdc_grid_spec."""
+    """Objects with .lo, .step, .n (5 each) and optionally .first (node offset per axis) -> array of cdc_grid_spec."""
     arr = (GridSpec * len(grids))()
     for i, g in enumerate(grids):
+        first = getattr(g, "first", None)
         for a in range(5):
             arr[i].lo[a] = float(g.lo[a]); arr[i].step[a] = float(g.step[a]); arr[i].n[a] = int(g.n[a])
+            arr[i].first[a] = 0 if first is None else int(first[a])
     return arr
 
 

@@ -53,6 +53,9 @@ extern "C" int32_t cdc_peel_turns(const cdc_geometry *g, cdc_events *ev, const c
     if (ev->geom != g) CDC_FAIL(CDC_ERR_INVALID, "cdc_peel_turns: events belong to another geometry");
     const int P = pp->max_partitions, E = ev->n_events;
     if (P < 1 || P > 8) CDC_FAIL(CDC_ERR_INVALID, "cdc_peel_turns: need 1 <= max_partitions <= 8");
+    for (int e = 0; e < ev->n_events; ++e)
+        for (int a = 0; a < 5; ++a)
+            if (h_grids0[e].first[a] != 0) CDC_FAIL(CDC_ERR_INVALID, "cdc_peel_turns: grid node offsets (first) must be 0");
     if (pp->min_hits < 0 || pp->min_classified < 0 || pp->extrap_max_steps < 1)
         CDC_FAIL(CDC_ERR_INVALID, "cdc_peel_turns: need min_hits >= 0, min_classified >= 0, extrap_max_steps >= 1");
     for (int a = 0; a < 5; ++a) {

@@ -42,6 +42,9 @@ extern "C" int32_t cdc_refine_tracks(const cdc_geometry *g, cdc_events *ev, cons
     if (ev->geom != g) CDC_FAIL(CDC_ERR_INVALID, "cdc_refine_tracks: events belong to another geometry");
     const int K = rp->n_parents, T = rp->n_iterations, E = ev->n_events;
     if (K < 1 || K > 8 || T < 0 || T > 20) CDC_FAIL(CDC_ERR_INVALID, "cdc_refine_tracks: need 1 <= n_parents <= 8, 0 <= n_iterations <= 20");
+    for (int e = 0; e < ev->n_events; ++e)
+        for (int a = 0; a < 5; ++a)
+            if (h_grids[e].first[a] != 0) CDC_FAIL(CDC_ERR_INVALID, "cdc_refine_tracks: grid node offsets (first) must be 0");
     cudaStream_t s = (cudaStream_t)stream;
     Dev D(s);
     int64_t total = 0;

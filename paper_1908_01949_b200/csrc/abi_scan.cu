@@ -67,6 +67,7 @@ int32_t prepare_grids(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec
             if (n < 1 || n > CDC_MAX_AXIS) CDC_FAIL(CDC_ERR_INVALID, "cdc_seed_scan: grid n must be in [1, 4096]");
             if (!isfinite(grids[e].lo[a]) || !isfinite(grids[e].step[a]))
                 CDC_FAIL(CDC_ERR_INVALID, "cdc_seed_scan: non-finite grid lo / step");
+            if (grids[e].first[a] < 0) CDC_FAIL(CDC_ERR_INVALID, "cdc_seed_scan: negative grid node offset (first)");
             prod *= n;
             if (prod > 2147483647LL) CDC_FAIL(CDC_ERR_INVALID, "cdc_seed_scan: more than 2^31 - 1 seeds in a grid");
             stride = std::max(stride, n);
@@ -98,12 +99,12 @@ int32_t prepare_grids(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec
         double *t = tab + (size_t)e * 6 * stride;
         const cdc_grid_spec &G = grids[e];
         for (int i = 0; i < G.n[0]; ++i) {            // reading C4: r0 = (R0 cos(theta), R0 sin(theta), z)
-            const double th = G.lo[0] + (double)i * G.step[0];
+            const double th = G.lo[0] + (double)(G.first[0] + i) * G.step[0];
             t[i] = g->R0 * cos(th);
             t[stride + i] = g->R0 * sin(th);
         }
         for (int a = 1; a < 5; ++a)
-            for (int i = 0; i < G.n[a]; ++i) t[(size_t)(a + 1) * stride + i] = G.lo[a] + (double)i * G.step[a];
+            for (int i = 0; i < G.n[a]; ++i) t[(size_t)(a + 1) * stride + i] = G.lo[a] + (double)(G.first[a] + i) * G.step[a];
         h_grids_pinned[e] = ev->h_grids[e];
     }
     const cudaError_t c1 = cudaMemcpyAsync(ev->axes.d, tab, sizeof(double) * n_tab, cudaMemcpyHostToDevice, s);

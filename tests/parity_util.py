@@ -35,24 +35,35 @@ def gpu_params(cfg, **kw):
     return B.scan_params(cfg.h_mm, cfg.max_steps, cfg.window_mm, cfg.eloss_MeV_per_mm, **kw)
 
 
-def explain_mismatch(bound, ev, seed, cfg, geom, dn=None, dchi2=None, same_track=False):
-    """Is a seed whose (n_match, n_steps) differ between the two sides one of the listed threshold classes?
-    dn, dchi2 (GPU minus oracle) and same_track (equal step and in-gas counts) make the test specific: when the two
-    tracks are the same and no approach sits at a wire end, the only listed class left is the window edge, and every
-    match gained or lost there carries resid^2 = lambda: the chi2 difference must be dn * lambda."""
+def explain_mismatch(bound, ev, seed, cfg, geom, dn=None, dchi2=None, same_track=False, gpu_steps=None, gpu_m_gas=None):
+    """Is a seed whose (n_match, n_steps, m_gas) differ between the two sides one of the listed threshold classes?
+    dn, dchi2 (GPU minus oracle) and same_track (equal step and in-gas counts) make the test specific:
+      * same track, no approach at a wire end: the only class left is the window edge, and every match gained or lost
+        there carries resid^2 = lambda, so the chi2 difference must be dn * lambda;
+      * different step / in-gas counts (gpu_steps, gpu_m_gas given): the threshold vertex must be WHERE THE TWO SIDES
+        DIVERGE, not anywhere on the track -- a differing in-gas count needs a vertex within 1e-3 mm of R0 no later than
+        the last vertex both sides reached (with energy loss every later difference follows from it); a differing step
+        count at equal in-gas count needs the vertex at which the shorter side stopped, min(n_steps), to lie within
+        1e-3 mm of an exit surface (|z| = z_half or rho = r_out)."""
     r = oracle.eval_seed(bound, ev.wire_id, ev.drift_mm, seed, records=True, rec_slack=0.1, trajectory=True)
     rec = r["rec"]
     edge_window = np.abs(np.abs(rec["resid"]) - cfg.window_mm) < EDGE_TOL_MM
     edge_zw = np.abs(np.abs(rec["zw"]) - geom.z_half_mm) < EDGE_TOL_MM
     traj = r["traj"]
     rho = np.hypot(traj[:, 0], traj[:, 1])
-    edge_exit = (np.abs(np.abs(traj[:, 2]) - geom.z_half_mm) < EDGE_TOL_MM).any() or \
-        (np.abs(rho - geom.r_out_mm) < EDGE_TOL_MM).any() or (np.abs(rho - geom.R0_mm) < EDGE_TOL_MM).any()
+    at_exit = (np.abs(np.abs(traj[:, 2]) - geom.z_half_mm) < EDGE_TOL_MM) | (np.abs(rho - geom.r_out_mm) < EDGE_TOL_MM)
+    at_R0 = np.abs(rho - geom.R0_mm) < EDGE_TOL_MM
     if same_track and dn is not None and dchi2 is not None and not edge_zw.any():
         lam = cfg.window_mm ** 2
         slack = abs(dn) * 4.0 * cfg.window_mm * EDGE_TOL_MM + 2e-3 * max(int(r["n_match"]), 1)   # edge width + fp32 chi2
         return bool(edge_window.any() and abs(dchi2 - dn * lam) <= slack)
-    return bool(edge_window.any() or edge_zw.any() or edge_exit)
+    if not same_track and gpu_steps is not None and gpu_m_gas is not None:
+        last_common = min(int(gpu_steps), int(r["n_steps"]))
+        if int(gpu_m_gas) != int(r["m_gas"]):
+            i0 = np.flatnonzero(at_R0)
+            return bool(i0.size and i0[0] <= last_common)
+        return bool(last_common < at_exit.size and at_exit[last_common])
+    return bool(edge_window.any() or edge_zw.any() or at_exit.any() or at_R0.any())
 
 
 def compare_scan(cfg, geom, field, ev, grid, gpu, orc, sel, offset=0):
@@ -73,7 +84,8 @@ def compare_scan(cfg, geom, field, ev, grid, gpu, orc, sel, offset=0):
     for i in bad:
         seed = grid.node(grid.unravel(int(sel[i])))
         assert explain_mismatch(bound, ev, seed, cfg, geom, dn=int(nm_g[i]) - int(orc["n_match"][i]),
-                                dchi2=float(c2_g[i]) - float(orc["chi2"][i]), same_track=bool(same_steps[i])), \
+                                dchi2=float(c2_g[i]) - float(orc["chi2"][i]), same_track=bool(same_steps[i]),
+                                gpu_steps=int(dbg["n_steps"][i]), gpu_m_gas=int(dbg["m_gas"][i])), \
             f"seed {int(sel[i])}: n_match {nm_g[i]} vs {orc['n_match'][i]}, steps {dbg['n_steps'][i]} vs " \
             f"{orc['n_steps'][i]} without a threshold case within {EDGE_TOL_MM} mm"
     assert len(bad) <= max(2, int(2e-3 * sel.size)), f"{len(bad)} threshold exceptions out of {sel.size}"

@@ -40,7 +40,7 @@ def test_library_is_sm100a_native_code():
 
 
 def test_struct_layouts_match_header():
-    assert C.sizeof(B.GridSpec) == 5 * 8 + 5 * 8 + 5 * 4 + 4          # padded to 8
+    assert C.sizeof(B.GridSpec) == 5 * 8 + 5 * 8 + 5 * 4 + 5 * 4
     assert C.sizeof(B.ScanParams) == 56
     assert C.sizeof(B.HoughParams) == 72
     assert C.sizeof(B.ScanStats) == 80

@@ -32,9 +32,10 @@ def test_theta_slabs_cover_the_grid_in_index_order():
     seen = []
     for r in range(3):
         sub, off = D.shard_theta(grid, r, 3)
+        assert np.array_equal(sub.lo, grid.lo) and int(sub.first[0]) == off // int(np.prod(grid.n[1:]))
         for lin in range(sub.n_seeds):
-            node = sub.node(sub.unravel(lin))
-            assert np.allclose(node, grid.node(grid.unravel(lin + off)), rtol=0, atol=1e-12)
+            node = D.slab_node(sub, sub.unravel(lin))                   # lo + (first + i) step, as the library forms it
+            assert np.array_equal(node, grid.node(grid.unravel(lin + off)))    # bit-identical to the full grid's node
             seen.append(lin + off)
     assert seen == list(range(grid.n_seeds))
     assert D.shard_theta(grid, 7, 8) == (None, 0)          # more ranks than theta nodes: empty slab
@@ -46,6 +47,17 @@ def test_globalize_and_unpack_keys():
     assert D.unpack_key(int(g[0])) == (3.5, 1007) and D.unpack_key(int(g[1])) == (0.0, 1000)
     # higher score wins; equal score -> lower index wins under MAX
     assert _pack([4.0], [9])[0] > _pack([3.5], [1])[0] and _pack([4.0], [2])[0] > _pack([4.0], [3])[0]
+
+
+def _fake_rank_result(rank, world, E, hit_offsets, seed=5):
+    """Per-rank 'exact winners' of a theta-sharded scan with many ties across ranks (same for every caller)."""
+    rng = np.random.default_rng(seed + rank)
+    nm = rng.integers(20, 24, size=E).astype(np.uint32)
+    chi2 = rng.integers(0, 3, size=E).astype(np.float64) * 0.25
+    seedidx = rng.integers(0, 50, size=E).astype(np.int64)
+    labels = rng.integers(-1, 3, size=int(hit_offsets[-1])).astype(np.int32)
+    offs = [rank * 1000 if (e + rank) % 4 != 3 else -1 for e in range(E)]          # some ranks own no slab of some events
+    return dict(best_seed=seedidx, best_n_match=nm, best_chi2=chi2, labels=labels), offs
 
 
 def _worker(rank, world, port, q):
@@ -63,6 +75,11 @@ def _worker(rank, world, port, q):
     q.put((rank, t.numpy().view(np.uint64).tolist()))
     # event sharding: ranks own disjoint event ranges, nothing to reduce
     q.put((rank, D.shard_range(E, rank, world)))
+    # the exact merge of a theta-sharded scan (fp64 S, lowest global index, owner's labels) as a collective
+    hit_offsets = np.array([0, 3, 7, 7, 12, 20, 21])
+    res, offs = _fake_rank_result(rank, world, 6, hit_offsets)
+    m = D.merge_slab_results_collective(res, offs, 1.0, hit_offsets)
+    q.put((rank, {k: m[k].tolist() for k in ("best_seed", "best_n_match", "best_chi2", "labels", "owner")}))
     dist.destroy_process_group()
 
 
@@ -72,7 +89,7 @@ def test_two_rank_key_reduction_equals_single_process_argmax():
     q = ctx.Queue()
     procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
     [p.start() for p in procs]
-    got = [q.get(timeout=120) for _ in range(4)]
+    got = [q.get(timeout=120) for _ in range(6)]
     [p.join(timeout=60) for p in procs]
     assert all(p.exitcode == 0 for p in procs)
     rng = np.random.default_rng(5)
@@ -83,3 +100,13 @@ def test_two_rank_key_reduction_equals_single_process_argmax():
     assert [D.unpack_key(k) for k in keys[0]] == want
     ranges = sorted(g[1] for g in got if isinstance(g[1], tuple))
     assert ranges == [(0, 2), (2, 4)]
+    # collective merge == the single-process merge of the same per-rank results, on both ranks
+    hit_offsets = np.array([0, 3, 7, 7, 12, 20, 21])
+    per_rank = [_fake_rank_result(r, 2, 6, hit_offsets) for r in range(2)]
+    ref = D.merge_slab_results([p[0] for p in per_rank], [p[1] for p in per_rank], 1.0, hit_offsets)
+    merged = [g[1] for g in got if isinstance(g[1], dict)]
+    assert len(merged) == 2
+    for m in merged:
+        for k in ("best_seed", "best_n_match", "best_chi2", "labels", "owner"):
+            assert m[k] == ref[k].tolist(), k
+    assert (ref["owner"] >= 0).all() and len(set(ref["owner"].tolist())) == 2          # both ranks win somewhere

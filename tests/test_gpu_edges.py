@@ -378,3 +378,37 @@ def test_candidate_pool_overflow_is_recovered_by_a_second_pass(setup, variant):
     fresh = sc.scan(E2, [g2], U.gpu_params(cfg, kernel_variant=variant), per_seed=False, debug=False)
     for key in ("best_seed", "best_n_match", "best_chi2", "labels", "best_key"):
         assert np.array_equal(again[key], fresh[key]), key
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_theta_sharded_scan_equals_the_unsharded_scan(setup, world):
+    """One event batch split over `world` GPUs along theta, the ranks run one after the
+    other on this one device: the merged best seed, chi2 (as doubles), n_match and labels must equal the unsharded call's,
+    bit for bit, and the slab node values must be bit-identical to the full grid's (the node offset travels in
+    cdc_grid_spec.first)."""
+    from paper_1908_01949_b200 import dist as D
+    cfg, geom, field, events, _, sc = setup
+    grids = [synth.truth_anchored_grid(ev.seed, (7, 6, 5, 5, 5))[0] for ev in events]     # 7 theta nodes: uneven slabs
+    grids[2] = synth.truth_anchored_grid(events[2].seed, (2, 6, 5, 5, 5))[0]              # fewer theta nodes than 3 ranks
+    off, w, d = synth.pack_hits(events)
+    P = U.gpu_params(cfg)
+    whole = sc.scan(sc.upload(off, w, d), grids, P, per_seed=False)
+    results, offsets = [], []
+    for rank in range(world):
+        subs, offs = sc.slabs(grids, rank, world)
+        for g, sub, o in zip(grids, subs, offs):
+            if o >= 0:
+                for i in range(int(sub.n[0])):
+                    lin = sub.linear((i, 0, 0, 0, 0))
+                    assert D.slab_node(sub, sub.unravel(lin))[0] == g.node(g.unravel(lin + o))[0]      # bit-identical
+        r = sc.scan_sharded(sc.upload(off, w, d), grids, P, rank, world, off, collective=False)
+        results.append(r["result"]); offsets.append(r["offsets"])
+    assert offsets[world - 1][2] == (-1 if world == 3 else offsets[world - 1][2])
+    merged = D.merge_slab_results(results, offsets, cfg.window_mm, off)
+    for k in ("best_seed", "best_n_match", "best_chi2", "labels"):
+        assert np.array_equal(merged[k], whole[k]), k
+    assert np.array_equal(merged["best_S"], D.exact_score(whole["best_n_match"], whole["best_chi2"], cfg.window_mm))
+    # the collective form of the merge in a single process (world size 1 degenerates to the rank's own result)
+    one = sc.scan_sharded(sc.upload(off, w, d), grids, P, 0, 1, off, collective=True)
+    for k in ("best_seed", "best_n_match", "best_chi2", "labels"):
+        assert np.array_equal(one[k], whole[k]), k
