@@ -57,6 +57,12 @@ def parse():
     ap.add_argument("--paper-mapping", action="store_true",
                     help="measure the re-created thread mapping of the paper (one block per seed, one thread per fired "
                          "wire) against the product kernel on a sample of the workload's seeds (comparison point)")
+    ap.add_argument("--issue-probe", action="store_true",
+                    help="issue rates of FFMA / FFMA2 / FADD2 / FMUL2 alone and mixed with integer work (the measurement "
+                         "behind the packed pairs of the scan kernel)")
+    ap.add_argument("--adaptive", action="store_true",
+                    help="SURVEY 8(f) #4: the adaptive-step scan against the fixed step on the workload: steps per seed, "
+                         "seeds/s, position difference (one JSON line per tolerance)")
     ap.add_argument("--peel", action="store_true",
                     help="measure the turn-partition peeling loop (cdc_peel_turns, SURVEY 8(f) #3) on the workload's "
                          "events: events/s, partitions found, efficiency / purity against the synthetic truth")
@@ -534,9 +540,61 @@ def run_peel(args):
                       "mean_purity": float(np.mean(pur)) if pur else None}))
 
 
+def run_issue_probe(args):
+    import torch
+    from paper_1908_01949_b200 import binding as B
+    torch.cuda.set_device(0)
+    names = ["FFMA", "FFMA2", "FADD", "FADD2", "FMUL2", "FFMA2 + LOP3", "FFMA + LOP3", "FFMA2 + FFMA"]
+    sm = torch.cuda.get_device_properties(0).multi_processor_count
+    for mode, name in enumerate(names):
+        ms, wi, fl = B.cdc_fp32_issue_probe(mode, 4096)
+        print(json.dumps({"probe": name, "ms": ms, "tflops": fl / ms * 1e-9,
+                          "warp_inst_per_clk_per_smsp_at_1965MHz": wi / (ms * 1e-3) / (sm * 4 * 1.965e9)}))
+
+
+def run_adaptive(args):
+    """Adaptive step against the fixed step on the same events and grids: kernel time, accepted steps per seed, and how
+    far the adaptive track ends from the fixed-step one (different path lengths by up to one long step are excluded:
+    only seeds that ended by the path cap at equal units are compared)."""
+    import torch
+    from paper_1908_01949_b200 import api, binding as B
+    torch.cuda.set_device(0)
+    args.events = args.events or (4 if args.workload == "cfg3" else 1)
+    cfg_id, cfg, geom, field, events, grids = make_workload(args, 0)
+    sc = api.SeedScanner(geom, field)
+    off, w, d = synth.pack_hits(events)
+    P = B.scan_params(cfg.h_mm, cfg.max_steps, cfg.window_mm, cfg.eloss_MeV_per_mm)
+    E = sc.upload(off, w, d)
+    fx = sc.scan(E, grids, P, per_seed=True, debug=True, best=False)
+    fx = sc.scan(E, grids, P, per_seed=True, debug=True, best=False)
+    n_seeds = fx["stats"]["n_seeds"]
+    print(json.dumps({"propagator": "fixed", "workload": args.workload, "events": len(events), "h_mm": cfg.h_mm,
+                      "kernel_ms": fx["stats"]["kernel_ms"], "seeds_per_s": n_seeds / (fx["stats"]["kernel_ms"] * 1e-3),
+                      "steps_per_seed": fx["stats"]["n_steps"] / n_seeds, "note": "TRACK variant (debug records on)"}))
+    for tol, h_max in ((1e-6, 8.0), (1e-5, 8.0), (1e-4, 8.0)):
+        ad = sc.scan_adaptive(E, grids, P, tol, h_max)
+        ad = sc.scan_adaptive(E, grids, P, tol, h_max)
+        same = ad["debug"]["pad"] == fx["debug"]["n_steps"]
+        dpos = np.sqrt(sum((ad["debug"][k] - fx["debug"][k]) ** 2 for k in ("x", "y", "z")))
+        dn = ad["n_match"].astype(np.int64) - fx["n_match"].astype(np.int64)
+        print(json.dumps({"propagator": "adaptive", "tol_mm": tol, "h_max_mm": h_max, "kernel_ms": ad["stats"]["kernel_ms"],
+                          "seeds_per_s": n_seeds / (ad["stats"]["kernel_ms"] * 1e-3),
+                          "steps_per_seed": ad["stats"]["n_steps"] / n_seeds,
+                          "path_units_per_seed": ad["stats"]["n_gas_steps"] / n_seeds,
+                          "steps_per_level": ad["n_level"].sum(axis=0).tolist(),
+                          "seeds_ending_at_equal_path": float(same.mean()),
+                          "max_position_difference_mm_at_equal_path": float(dpos[same].max()) if same.any() else None,
+                          "n_match_differs_on_fraction": float((dn != 0).mean()),
+                          "best_seed_same": bool(np.array_equal(ad["S32_argmax"], fx["S32_argmax"]))}))
+
+
 if __name__ == "__main__":
     a = parse()
-    if a.peel:
+    if a.issue_probe:
+        run_issue_probe(a)
+    elif a.adaptive:
+        run_adaptive(a)
+    elif a.peel:
         run_peel(a)
     elif a.paper_mapping:
         run_paper_mapping(a)

@@ -169,6 +169,22 @@ int32_t cdc_hough_seed_ranges(const cdc_geometry *g, const cdc_events *ev, const
 int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec *h_grids,
                       const cdc_scan_params *params, uint32_t *d_n_match_or_null, float *d_chi2_or_null,
                       cdc_seed_debug *d_debug_or_null, uint64_t *d_best_key, void *stream);
+/* the seed scan with the ADAPTIVE step of the propagator the paper cites ("the RKN method
+ * was used for the track parameter propagation [5]"; [5] = Lund et al.; reading C19 applied to the scan).
+ * Step lengths h 2^j with h 2^j <= h_max_mm; a trial whose error estimate H^2 max|k1 - k2 - k3 + k4| exceeds tol_mm is
+ * repeated one level down (never below h), an accepted step with estimate <= tol / 32 raises the level of the next
+ * trial.  params->max_steps caps the PATH in units of h; the in-gas count and the energy loss are in those units.
+ * Outputs per seed (device, caller-owned): d_n_match u32, d_chi2 f32 (either may be NULL), d_debug_or_null (n_steps =
+ * accepted steps, m_gas = in-gas path units, pad = path units, final position), d_levels_or_null i32 [seeds][8]
+ * (accepted steps per level 0..6; [7] = hash of the level sequence, hash = hash * 31 + (level + 1)); d_best_key per
+ * event: the fused fp32 arg max, packed as cdc_seed_scan packs it.  The step-size decisions are taken in fp32: a seed
+ * whose estimate comes within ~2 % of a threshold can take another sequence than an fp64 evaluation (DESIGN.md
+ * section 15).  No candidate pool is filled: cdc_best_track does not apply.  h_max is limited by the 2 x 2 wire lookup
+ * (CDC_ERR_RANGE above ~12 mm).  Asynchronous. */
+int32_t cdc_seed_scan_adaptive(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec *h_grids,
+                               const cdc_scan_params *params, double tol_mm, double h_max_mm, uint32_t *d_n_match_or_null,
+                               float *d_chi2_or_null, cdc_seed_debug *d_debug_or_null, int32_t *d_levels_or_null,
+                               uint64_t *d_best_key, void *stream);
 /* Counters of the last scan.  Synchronises `stream`. */
 int32_t cdc_scan_get_stats(const cdc_events *ev, cdc_scan_stats *h_out, void *stream);
 
@@ -292,6 +308,14 @@ uint64_t cdc_kernel_launch_count(void);
 /* Register-only FFMA chain: the empirical FP32 peak used as the roofline denominator.  Runs `iters`
  * dependent-chain iterations on every SM, returns achieved FLOP/s (2 per FFMA).  Synchronises. */
 int32_t cdc_fp32_peak_probe(int32_t iters, double *h_flops_per_s, double *h_ms, void *stream);
+
+/* Issue rates of sm_100a's packed fp32 instructions (PTX fma/add/mul.rn.f32x2 -> SASS FFMA2/FADD2/FMUL2) against the
+ * scalar ones, alone and interleaved with integer-pipe work: register-only chains on every SM.  mode: 0 FFMA, 1 FFMA2,
+ * 2 FADD, 3 FADD2, 4 FMUL2, 5 FFMA2 + LOP3, 6 FFMA + LOP3, 7 FFMA2 + FFMA.  Returns the kernel time, the warp
+ * instructions and the flops it executed (the measurement behind the packed pairs of the scan kernel, DESIGN.md
+ * section 7; `python bench.py --issue-probe`).  Synchronises. */
+int32_t cdc_fp32_issue_probe(int32_t mode, int32_t iters, double *h_ms, double *h_warp_instructions, double *h_flops,
+                             void *stream);
 
 #ifdef __cplusplus
 }

@@ -78,6 +78,27 @@ class SeedScanner:
             out["debug"] = d_dbg.cpu().numpy().view(B.SEED_DEBUG_DTYPE)
         return out
 
+    def scan_adaptive(self, events: B.Events, grids: Sequence, params: B.ScanParams, tol_mm: float, h_max_mm: float) -> dict:
+        """cdc_seed_scan_adaptive with every per-seed output; numpy arrays concatenated over events."""
+        torch = _torch()
+        E = events.n_events
+        n_seeds = [int(np.prod(np.asarray(g.n, dtype=np.int64))) for g in grids]
+        total = int(sum(n_seeds))
+        d_key = torch.zeros(E, dtype=torch.int64, device="cuda")
+        d_nm = torch.zeros(total, dtype=torch.int32, device="cuda"); d_c2 = torch.zeros(total, dtype=torch.float32, device="cuda")
+        d_dbg = torch.zeros(total * B.SEED_DEBUG_DTYPE.itemsize, dtype=torch.uint8, device="cuda")
+        d_lev = torch.zeros((total, 8), dtype=torch.int32, device="cuda")
+        B.cdc_seed_scan_adaptive(self.geometry, events, B.grid_specs(grids), params, tol_mm, h_max_mm, d_key, d_nm, d_c2,
+                                 d_dbg, d_lev)
+        torch.cuda.synchronize()
+        key = d_key.cpu().numpy().view(np.uint64)
+        lev = d_lev.cpu().numpy()
+        return dict(n_seeds=n_seeds, n_match=d_nm.cpu().numpy().astype(np.uint32), chi2=d_c2.cpu().numpy(),
+                    debug=d_dbg.cpu().numpy().view(B.SEED_DEBUG_DTYPE), n_level=lev[:, :7], seq_hash=lev[:, 7].view(np.uint32),
+                    best_key=key, S32_max=(key >> np.uint64(32)).astype(np.uint32).view(np.float32),
+                    S32_argmax=(np.uint64(0xFFFFFFFF) - (key & np.uint64(0xFFFFFFFF))).astype(np.int64),
+                    stats=B.cdc_scan_get_stats(events))
+
     def slabs(self, grids: Sequence, rank: int, world: int):
         """This rank's theta slab of every grid (dist.shard_theta) and the index offsets back to the full grids; an
         event whose theta axis has fewer nodes than ranks gets a one-node placeholder here and offset -1 (ignored)."""

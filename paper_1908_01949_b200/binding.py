@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(HERE, "libcdc_seedscan.so")
 EXPORTS = ["cdc_last_error", "cdc_geometry_create", "cdc_geometry_destroy", "cdc_geometry_wire_table",
            "cdc_event_upload", "cdc_events_destroy", "cdc_events_tables", "cdc_hough_dims",
            "cdc_hough_seed_ranges", "cdc_seed_scan", "cdc_scan_get_stats", "cdc_best_track",
-           "cdc_find_tracks_host", "cdc_refine_tracks", "cdc_peel_turns", "cdc_classification_quality", "cdc_common_hits", "cdc_seed_scan_paper_mapping", "cdc_seed_scan_paper_mapping_v2", "cdc_fp32_peak_probe", "cdc_kernel_launch_count"]
+           "cdc_find_tracks_host", "cdc_refine_tracks", "cdc_peel_turns", "cdc_classification_quality", "cdc_common_hits", "cdc_seed_scan_paper_mapping", "cdc_seed_scan_paper_mapping_v2", "cdc_seed_scan_adaptive", "cdc_fp32_peak_probe", "cdc_fp32_issue_probe", "cdc_kernel_launch_count"]
 
 
 class CdcError(RuntimeError):
@@ -246,6 +246,15 @@ def cdc_best_track(geometry: Geometry, events: Events, grids: C.Array, params: S
                                 _stream(stream)))
 
 
+def cdc_seed_scan_adaptive(geometry: Geometry, events: Events, grids: C.Array, params: ScanParams, tol_mm: float,
+                           h_max_mm: float, d_best_key, d_n_match=None, d_chi2=None, d_debug=None, d_levels=None,
+                           stream=None) -> None:
+    """SURVEY 8(f) #4: the scan with the adaptive RKN step (device outputs, caller-owned torch tensors)."""
+    _check(lib().cdc_seed_scan_adaptive(geometry.handle, events.handle, grids, C.byref(params), C.c_double(tol_mm),
+                                        C.c_double(h_max_mm), _dp(d_n_match), _dp(d_chi2), _dp(d_debug), _dp(d_levels),
+                                        _dp(d_best_key), _stream(stream)))
+
+
 def cdc_find_tracks_host(geometry: Geometry, hit_offsets, wire_id, drift_mm, grids: C.Array, params: ScanParams,
                          hp: Optional[HoughParams] = None, zref=None, hough_sets_axes: bool = True, stream=None) -> dict:
     """End-to-end call with host (numpy) buffers in and out.  With hp the Hough vote runs; its ranges replace the
@@ -343,6 +352,12 @@ def cdc_seed_scan_paper_mapping_v2(geometry: Geometry, events: Events, event: in
 
 def cdc_kernel_launch_count() -> int:
     return int(lib().cdc_kernel_launch_count())
+
+
+def cdc_fp32_issue_probe(mode: int, iters: int = 4096, stream=None):
+    ms = C.c_double(); wi = C.c_double(); fl = C.c_double()
+    _check(lib().cdc_fp32_issue_probe(C.c_int32(mode), C.c_int32(iters), C.byref(ms), C.byref(wi), C.byref(fl), _stream(stream)))
+    return float(ms.value), float(wi.value), float(fl.value)
 
 
 def cdc_fp32_peak_probe(iters: int = 4096, stream=None):

@@ -259,7 +259,46 @@ extern "C" int32_t cdc_seed_scan(const cdc_geometry *g, cdc_events *ev, const cd
     L.d_n_match = d_n_match; L.d_chi2 = d_chi2; L.d_debug = d_debug; L.d_best_key = d_best_key;
     if (!ev->ev_k0) { CDC_CUDA(cudaEventCreate(&ev->ev_k0)); CDC_CUDA(cudaEventCreate(&ev->ev_k1)); }
     CDC_CUDA(launch_seed_scan(L, s, ev->ev_k0, ev->ev_k1));
-    ev->scanned = true;
+    ev->scanned = true; ev->adaptive_scanned = false;
+    ev->last_stream = s;
+    return CDC_OK;
+    });
+}
+
+// ------------------------------------------------------------------------------------------------ SURVEY 8(f) #4
+extern "C" int32_t cdc_seed_scan_adaptive(const cdc_geometry *g, cdc_events *ev, const cdc_grid_spec *h_grids,
+                                          const cdc_scan_params *p, double tol_mm, double h_max_mm, uint32_t *d_n_match,
+                                          float *d_chi2, cdc_seed_debug *d_debug, int32_t *d_levels, uint64_t *d_best_key,
+                                          void *stream)
+{
+    return cdc_guard("cdc_seed_scan_adaptive", [&]() -> int32_t {
+    if (!g || !ev || !h_grids || !d_best_key) CDC_FAIL(CDC_ERR_INVALID, "cdc_seed_scan_adaptive: null argument");
+    if (ev->geom != g) CDC_FAIL(CDC_ERR_INVALID, "cdc_seed_scan_adaptive: events belong to another geometry");
+    int32_t rc = check_params(p, "cdc_seed_scan_adaptive");
+    if (rc != CDC_OK) return rc;
+    if (!(tol_mm > 0.0) || !isfinite(tol_mm) || !(h_max_mm >= p->h_mm) || !isfinite(h_max_mm))
+        CDC_FAIL(CDC_ERR_INVALID, "cdc_seed_scan_adaptive: need tol > 0 and h_max >= h");
+    int J = 0;
+    while (J < 6 && p->h_mm * (double)(2 << J) <= h_max_mm) ++J;            // levels 0 .. J, h 2^J <= h_max
+    const double H = p->h_mm * (double)(1 << J);
+    // the 2 x 2 set around a step's START vertex must hold every wire that can own a match in that step
+    const double dmax = 8.0 + p->window_mm + 0.05;
+    const double reach = sqrt(dmax * dmax + H * H) + 0.1;
+    if (reach > g->excl) CDC_FAIL(CDC_ERR_RANGE, "cdc_seed_scan_adaptive: window + longest step too large for the 2 x 2 wire lookup (h_max <= ~12 mm)");
+    cudaStream_t s = (cudaStream_t)stream;
+    if ((rc = prepare_grids(g, ev, h_grids, s)) != CDC_OK) return rc;
+    CDC_CUDA(cudaMemsetAsync(d_best_key, 0, sizeof(uint64_t) * (size_t)ev->n_events, s));
+    CDC_CUDA(cudaMemsetAsync(ev->d_counters, 0, sizeof(unsigned long long) * CNT_N, s));
+    ScanLaunch L;
+    if ((rc = fill_scan_launch(g, ev, p, L)) != CDC_OK) return rc;
+    L.d_n_match = d_n_match; L.d_chi2 = d_chi2; L.d_debug = d_debug; L.d_best_key = d_best_key;
+    const double grow = reach + 0.2;
+    const double ulo = std::max(g->r[0] - grow, 0.0), uhi = g->r[g->n_layers - 1] + grow;
+    L.u2_lo = (float)(ulo * ulo); L.u2_hi = (float)(uhi * uhi);
+    if (!ev->ev_k0) { CDC_CUDA(cudaEventCreate(&ev->ev_k0)); CDC_CUDA(cudaEventCreate(&ev->ev_k1)); }
+    CDC_CUDA(launch_seed_scan_adaptive(L, tol_mm, J, d_levels, s, ev->ev_k0, ev->ev_k1));
+    ev->scanned = false;                       // no candidate pool was filled: cdc_best_track does not apply to this variant
+    ev->adaptive_scanned = true;
     ev->last_stream = s;
     return CDC_OK;
     });
@@ -269,7 +308,7 @@ extern "C" int32_t cdc_scan_get_stats(const cdc_events *ev, cdc_scan_stats *out,
 {
     return cdc_guard("cdc_scan_get_stats", [&]() -> int32_t {
     if (!ev || !out) CDC_FAIL(CDC_ERR_INVALID, "cdc_scan_get_stats: null argument");
-    if (!ev->scanned) CDC_FAIL(CDC_ERR_NOT_READY, "cdc_scan_get_stats: no scan has run on these events");
+    if (!ev->scanned && !ev->adaptive_scanned) CDC_FAIL(CDC_ERR_NOT_READY, "cdc_scan_get_stats: no scan has run on these events");
     unsigned long long c[CNT_N];
     CDC_CUDA(cudaMemcpyAsync(c, ev->d_counters, sizeof(c), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
     CDC_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
@@ -372,6 +411,16 @@ extern "C" int32_t cdc_fp32_peak_probe(int32_t iters, double *h_flops_per_s, dou
     return cdc_guard("cdc_fp32_peak_probe", [&]() -> int32_t {
     if (iters < 1) CDC_FAIL(CDC_ERR_INVALID, "cdc_fp32_peak_probe: iters < 1");
     CDC_CUDA(run_fp32_peak_probe(iters, h_flops_per_s, h_ms, (cudaStream_t)stream));
+    return CDC_OK;
+    });
+}
+
+extern "C" int32_t cdc_fp32_issue_probe(int32_t mode, int32_t iters, double *h_ms, double *h_warp_instructions, double *h_flops,
+                                        void *stream)
+{
+    return cdc_guard("cdc_fp32_issue_probe", [&]() -> int32_t {
+    if (iters < 1 || mode < 0 || mode > 7) CDC_FAIL(CDC_ERR_INVALID, "cdc_fp32_issue_probe: need iters >= 1, 0 <= mode <= 7");
+    CDC_CUDA(run_fp32_issue_probe(mode, iters, h_ms, h_warp_instructions, h_flops, (cudaStream_t)stream));
     return CDC_OK;
     });
 }

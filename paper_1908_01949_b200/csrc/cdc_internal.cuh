@@ -127,6 +127,7 @@ struct cdc_events {
     uint32_t pool_cap = 0;
     unsigned long long *d_counters = nullptr;   // [8]: steps, gas steps, approach tests, pool count, ...
     bool scanned = false;
+    bool adaptive_scanned = false;           // the last scan was cdc_seed_scan_adaptive (counters: steps, path units)
     cudaEvent_t ev_k0 = nullptr, ev_k1 = nullptr;   // bracket of the scan kernel
     // best-track scratch
     double *d_pool_S64 = nullptr, *d_pool_chi2 = nullptr;
@@ -220,6 +221,8 @@ struct ScanLaunch {
                                          // largest half-separation (as a wire sees it) served by one shared lookup
 };
 cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0, cudaEvent_t k1);
+cudaError_t launch_seed_scan_adaptive(const ScanLaunch &L, double tol, int J, int32_t *d_levels, cudaStream_t s, cudaEvent_t k0,
+                                      cudaEvent_t k1);
 
 cudaError_t launch_bin_events(int32_t n_events, int32_t W, int32_t n_bit_words, int32_t max_hits_per_event,
                               const int32_t *d_offsets, const int32_t *d_wire_id, const float *d_drift,
@@ -276,3 +279,4 @@ cudaError_t launch_best_track(const BestLaunch &L, cudaStream_t s);
 int32_t cdc_lookup_every64(const cdc_geometry *g, double h_mm, double window_mm);
 
 cudaError_t run_fp32_peak_probe(int32_t iters, double *flops_per_s, double *ms, cudaStream_t s);
+cudaError_t run_fp32_issue_probe(int32_t mode, int32_t iters, double *ms_out, double *warp_inst, double *flops, cudaStream_t s);

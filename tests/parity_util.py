@@ -5,7 +5,8 @@ Tolerances (BASELINE.json north_star):
   * propagated positions agree within 1e-3 mm after the full track (at equal step count);
   * per-seed matched-hit counts identical, except hits whose distance lies within 1e-3 mm of the window edge
     (and the sibling threshold classes of DESIGN.md section 6: |z_w| within 1e-3 of the wire end, a vertex within
-    1e-3 mm of an exit surface) -- each such seed is listed and counted;
+    1e-3 mm of an exit surface or of R0, an approach whose foot lies within 1e-3 mm of the track's first / last vertex
+    or of a vertex where the in-gas flag changes) -- each such seed is listed and counted;
   * best seed and hit -> turn labels bit-exact (n_match and chi2 of the best seed bit-equal as doubles).
 """
 import numpy as np
@@ -56,7 +57,31 @@ def explain_mismatch(bound, ev, seed, cfg, geom, dn=None, dchi2=None, same_track
     if same_track and dn is not None and dchi2 is not None and not edge_zw.any():
         lam = cfg.window_mm ** 2
         slack = abs(dn) * 4.0 * cfg.window_mm * EDGE_TOL_MM + 2e-3 * max(int(r["n_match"]), 1)   # edge width + fp32 chi2
-        return bool(edge_window.any() and abs(dchi2 - dn * lam) <= slack)
+        if edge_window.any() and abs(dchi2 - dn * lam) <= slack:
+            return True
+        # Ownership at a boundary vertex: interval n owns an approach iff g_n <= 0 < g_{n+1} (reading C9).  Where g is
+        # within 1e-3 mm of zero AT a vertex the two sides may hand the approach to different intervals -- harmless
+        # between two scored intervals, but at the track's last or first vertex, or where the in-gas flag changes,
+        # the interval on the other side does not exist or is not scored: the match (with its resid^2, the distance of
+        # that very vertex to the wire) is gained or lost.
+        gas = (rho >= geom.R0_mm); gas[0] = True
+        nv = traj.shape[0] - 1
+        boundary = sorted({0, nv} | set(np.flatnonzero(gas[1:] != gas[:-1]) + 1))
+        wires = geom.wire[ev.wire_id].astype(np.float64)
+        cand = []
+        for v in boundary:
+            pos, T = traj[v, :3], traj[v, 3:]
+            dvec = pos[None, :] - np.concatenate([wires[:, :2], np.zeros((wires.shape[0], 1))], axis=1)
+            u = wires[:, 2:5]
+            delta = dvec - (dvec * u).sum(axis=1)[:, None] * u
+            g = delta @ T
+            D = np.linalg.norm(delta, axis=1)
+            for k in np.flatnonzero(np.abs(g) < EDGE_TOL_MM):
+                cand.append((D[k] - float(ev.drift_mm[k])) ** 2)
+        cand = [c for c in cand if c < lam * 1.01]
+        if abs(dn) == 1 and any(abs(abs(dchi2) - c) <= slack for c in cand) and np.sign(dchi2) == np.sign(dn):
+            return True
+        return False
     if not same_track and gpu_steps is not None and gpu_m_gas is not None:
         last_common = min(int(gpu_steps), int(r["n_steps"]))
         if int(gpu_m_gas) != int(r["m_gas"]):
