@@ -175,7 +175,10 @@ extern "C" int32_t cdc_geometry_create(const cdc_geometry_desc *gd, const cdc_fi
         // per-cell bilinear coefficients for the fp32 scan, taken about the CELL CENTRE:
         //   B(wr, wz) = c0 + c_r wr + c_z wz + c_rz wr wz,  wr, wz in [-1/2, 1/2] = offset from the centre in cell units
         // (combinations of the fp32 node values formed in fp64, rounded once), stored as (c0, c_z, c_r, c_rz): the two
-        // register pairs of one 128-bit load are then the operands of ONE packed FMA, (c0, c_z) + wr (c_r, c_rz)
+        // register pairs of one 128-bit load are then the operands of ONE packed FMA, (c0, c_z) + wr (c_r, c_rz).
+        // Cell (ir, iz) is record ir (nz - 1) + iz: z runs fastest, because the 32 tracks of a warp differ in z0 first
+        // (same rho, a spread of z): their cells are then neighbours in memory and one gather touches 2-3 lines
+        // instead of one line per track (the L1 data pipe was 70 % busy with [iz][ir], ncu r2)
         const int ncr = fd->nr - 1, ncz = fd->nz - 1;
         std::vector<float4> cells((size_t)ncr * ncz * 2);
         for (int iz = 0; iz < ncz; ++iz)
@@ -186,7 +189,7 @@ extern "C" int32_t cdc_geometry_create(const cdc_geometry_desc *gd, const cdc_fi
                     const double n10 = g->field_tab[((size_t)(iz + 1) * fd->nr + ir) * 2 + c];
                     const double n11 = g->field_tab[((size_t)(iz + 1) * fd->nr + ir + 1) * 2 + c];
                     const double crz = n11 - n10 - n01 + n00;
-                    cells[((size_t)iz * ncr + ir) * 2 + c] =
+                    cells[((size_t)ir * ncz + iz) * 2 + c] =
                         make_float4((float)(0.25 * (n00 + n01 + n10 + n11)), (float)((n10 - n00) + 0.5 * crz),
                                     (float)((n01 - n00) + 0.5 * crz), (float)crz);
                 }

@@ -35,7 +35,7 @@ struct FieldDev {
     float cr, cz;            // -r0 / dr - 1/2, -z0 / dz - 1/2: fma(rho, inv_dr, cr) = cell coordinate - 1/2
     int32_t n_cells;         // (nr - 1) (nz - 1)
     const float2 *tab;       // [nz][nr] (B_r, B_z) nodes (fp64 path)
-    const float4 *cells;     // [nz-1][nr-1][2]: bilinear coefficients about the cell centre (c0, c_z, c_r, c_rz) of B_r, then of B_z
+    const float4 *cells;     // [nr-1][nz-1][2] (z fastest): bilinear coefficients about the cell centre (c0, c_z, c_r, c_rz) of B_r, then of B_z
 };
 
 struct GeomDev {

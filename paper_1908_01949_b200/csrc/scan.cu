@@ -154,7 +154,8 @@ __device__ __forceinline__ void field_at_p(const FieldDev &F, f2 xy, float z, f2
     const f2 t = add2(f, kMagicRound);
     const f2 w = sub2(f, sub2(t, kMagicRound));                                     // offsets from the cell centre
     const int ir = __float_as_int(lo(t)) - kMagicRoundBits, iz = __float_as_int(hi(t)) - kMagicRoundBits;
-    const unsigned cell = min((unsigned)(iz * (F.nr - 1) + ir), (unsigned)(F.n_cells - 1));
+    const unsigned cell = min((unsigned)(ir * (F.nz - 1) + iz), (unsigned)(F.n_cells - 1));
+    // (keeping the cell's coefficients in registers and loading only on a cell change was measured: no gain, r2)
     const float4 *c = F.cells + 2u * cell;
     const float4 cr = __ldg(c), cz = __ldg(c + 1);                                  // (c0, c_z, c_r, c_rz) of B_r, of B_z
     const f2 tr = fma2(bc(lo(w)), pk(cr.z, cr.w), pk(cr.x, cr.y)), tz = fma2(bc(lo(w)), pk(cz.z, cz.w), pk(cz.x, cz.y));

@@ -60,7 +60,7 @@ __device__ __forceinline__ void field_at(const FieldDev &F, float x, float y, fl
         const float tr = fr + kMagicRound, tz = fz + kMagicRound;
         const float wr = fr - (tr - kMagicRound), wz = fz - (tz - kMagicRound);
         const int ir = __float_as_int(tr) - kMagicRoundBits, iz = __float_as_int(tz) - kMagicRoundBits;
-        const unsigned cell = min((unsigned)(iz * (F.nr - 1) + ir), (unsigned)(F.n_cells - 1));
+        const unsigned cell = min((unsigned)(ir * (F.nz - 1) + iz), (unsigned)(F.n_cells - 1));
         const float4 *c = F.cells + 2u * cell;
         const float4 cr = __ldg(c), cz = __ldg(c + 1);                   // (c0, c_z, c_r, c_rz) of B_r, of B_z
         const float Br = fmaf(wz, fmaf(wr, cr.w, cr.y), fmaf(wr, cr.z, cr.x));

@@ -173,10 +173,10 @@ __device__ __forceinline__ void field_at2(const FieldDev &F, f2 x, f2 y, f2 z, f
     const f2 fr = fma2(rho, bc(F.inv_dr), bc(F.cr)), fz = fma2(z, bc(F.inv_dz), bc(F.cz));      // cell coordinate - 1/2
     const f2 tr = add2(fr, kMagicRound), tz = add2(fz, kMagicRound);
     const f2 wr = sub2(fr, sub2(tr, kMagicRound)), wz = sub2(fz, sub2(tz, kMagicRound));
-    const int nrc = F.nr - 1;
-    const unsigned cellA = min((unsigned)((__float_as_int(lo(tz)) - kMagicRoundBits) * nrc + (__float_as_int(lo(tr)) - kMagicRoundBits)),
+    const int nzc = F.nz - 1;
+    const unsigned cellA = min((unsigned)((__float_as_int(lo(tr)) - kMagicRoundBits) * nzc + (__float_as_int(lo(tz)) - kMagicRoundBits)),
                                (unsigned)(F.n_cells - 1));
-    const unsigned cellB = min((unsigned)((__float_as_int(hi(tz)) - kMagicRoundBits) * nrc + (__float_as_int(hi(tr)) - kMagicRoundBits)),
+    const unsigned cellB = min((unsigned)((__float_as_int(hi(tr)) - kMagicRoundBits) * nzc + (__float_as_int(hi(tz)) - kMagicRoundBits)),
                                (unsigned)(F.n_cells - 1));
     const float4 *cA = F.cells + 2u * cellA, *cB = F.cells + 2u * cellB;
     const float4 rA = __ldg(cA), zA = __ldg(cA + 1), rB = __ldg(cB), zB = __ldg(cB + 1);
