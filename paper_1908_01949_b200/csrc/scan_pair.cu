@@ -1,4 +1,7 @@
-// A3-A7, the production form: TWO seeds per thread, arithmetic in packed fp32 pairs (pair_math.cuh).
+// A3-A7, the COMPARISON variant (params.kernel_variant = 1): TWO seeds per thread, arithmetic in packed fp32 pairs
+// (pair_math.cuh).  Measured slower than the one-seed kernel of scan.cu on B200 (profiles/r2_pair_kernel.md: fewer
+// instructions per seed, but 128 / 94 registers, 16 / 20 warps per SM, and the FP32 pipe time is unchanged by packing);
+// kept, tested (tests/test_gpu_pair.py), as the measured answer to "carry pairs in f32x2".
 //
 // The two seeds of a thread are neighbours on the z0 axis of the grid: same theta, px, py, pz, hence the same start
 // point in (x, y), the same momentum p (one curvature constant a = kappa q / p for both) and the same start direction.
@@ -8,7 +11,8 @@
 //     three field evaluations, the stage derivatives and the updates are packed pairs -- every FFMA2 / FADD2 / FMUL2 is one
 //     issue slot for both seeds.
 // Every half of a packed instruction rounds like the scalar instruction, and the operation order is that of the
-// one-seed kernel (scan.cu), so per-seed results are identical to it; tests/test_gpu_pair.py compares them bit for bit.
+// one-seed kernel (scan.cu), so per-seed match counts, step counts, the exact best seed and the labels are identical to
+// its results (tests/test_gpu_pair.py).
 //
 //   PAPER.md:51      seed (theta0, z0, px0, py0, pz0) at R0                     -> prologue
 //   PAPER.md:55      RKN propagation (textbook Nystroem scheme, reading C5)     -> step body
