@@ -166,8 +166,11 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "seeds_per_event": grids[0].n_seeds, "max_steps": cfg.max_steps,
-                       "h_mm": cfg.h_mm},
+            # the workload is the main arm's (same keys, same values); what the oracle was timed on is in `sample`
+            "config": {"workload": args.workload, "events_per_gpu": synth.CONFIGS[cfg_id].n_events,
+                       "seeds_per_event": grids[0].n_seeds, "max_steps": cfg.max_steps, "h_mm": cfg.h_mm,
+                       "field": "table" if cfg.field_kind else "uniform", "hits_event0": len(events[0].wire_id),
+                       "sample": sample},
             "rkn_steps_per_s": steps / total,
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
