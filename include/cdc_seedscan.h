@@ -86,7 +86,12 @@ typedef struct {
  * kernel_variant: 0 = the production kernel (one seed per thread; (x, y) components as packed fp32 pairs);
  *   1 = two z0-neighbour seeds per thread, every quantity a packed pair of the two seeds (csrc/scan_pair.cu): measured
  *   slower on B200 (profiles/r2_pair_kernel.md), kept as the comparison point; per-seed n_match,
- *   step counts, best seed and labels are identical, tests/test_gpu_pair.py checks it. */
+ *   step counts, best seed and labels are identical, tests/test_gpu_pair.py checks it;
+ *   2 = lane refill (csrc/scan_refill.cu): a thread runs two seeds in a row, the short track of one 32-seed chunk and
+ *   the long track of the next, and a per-step warp vote ends the warp: every lane stays live (32.0 of 32 in the step
+ *   against 29.3 / 30.8) but the second seeds are out of step with their z0 neighbours and the lookup and live-wire
+ *   code pay more than the step saves: measured slower (profiles/r2_refill_kernel.md), kept as the comparison point;
+ *   per-seed n_match, chi2, positions, best seed and labels are bit-identical, tests/test_gpu_refill.py checks it. */
 typedef struct {
     double h_mm;
     int32_t max_steps;

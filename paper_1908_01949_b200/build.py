@@ -13,11 +13,11 @@ ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC,-ffp-contract=off,-Wall", *ARCH]
 SOURCES = {                      # file -> extra flags
     "abi.cu": [], "abi_events.cu": [], "abi_scan.cu": [], "abi_e2e.cu": [],
-    "events.cu": [], "hough.cu": [], "scan.cu": ["-Xptxas", "-v"], "scan_pair.cu": ["-Xptxas", "-v"], "scan_adaptive.cu": [], "peak.cu": [],
+    "events.cu": [], "hough.cu": [], "scan.cu": ["-Xptxas", "-v"], "scan_pair.cu": ["-Xptxas", "-v"], "scan_refill.cu": ["-Xptxas", "-v"], "scan_adaptive.cu": [], "peak.cu": [],
     "best.cu": ["-fmad=false"], "refine.cu": ["-fmad=false"], "abi_refine.cu": [], "quality.cu": [], "paper_v1.cu": [], "paper_v2.cu": [],
     "peel.cu": ["-fmad=false"], "abi_peel.cu": [],
 }
-HEADERS = [os.path.join(CSRC, "paper_common.cuh"), os.path.join(CSRC, "peel.cuh"), os.path.join(CSRC, "refine.cuh"), os.path.join(CSRC, "cdc_internal.cuh"), os.path.join(CSRC, "eval64.cuh"), os.path.join(CSRC, "scan_common.cuh"), os.path.join(CSRC, "scan_args.cuh"), os.path.join(CSRC, "pair_math.cuh"), os.path.join(HERE, "..", "include", "cdc_seedscan.h")]
+HEADERS = [os.path.join(CSRC, "paper_common.cuh"), os.path.join(CSRC, "peel.cuh"), os.path.join(CSRC, "refine.cuh"), os.path.join(CSRC, "cdc_internal.cuh"), os.path.join(CSRC, "eval64.cuh"), os.path.join(CSRC, "scan_common.cuh"), os.path.join(CSRC, "scan_args.cuh"), os.path.join(CSRC, "pair_math.cuh"), os.path.join(CSRC, "scan_one.cuh"), os.path.join(HERE, "..", "include", "cdc_seedscan.h")]
 
 
 def _stale(target, deps):

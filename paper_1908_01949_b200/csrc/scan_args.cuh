@@ -1,4 +1,5 @@
-// Kernel arguments of the seed-scan kernels (scan.cu: one seed per thread; scan_pair.cu: two seeds per thread).
+// Kernel arguments of the seed-scan kernels (scan.cu: one seed per thread; scan_pair.cu: two seeds per thread;
+// scan_refill.cu: one seed per thread at a time, two in a row).
 #pragma once
 #include "cdc_internal.cuh"
 
@@ -38,3 +39,4 @@ struct ScanArgs {
 };
 
 cudaError_t launch_seed_scan_pair(const ScanArgs &A, const ScanLaunch &L, bool eloss, bool track, cudaStream_t s);
+cudaError_t launch_seed_scan_refill(const ScanArgs &A, const ScanLaunch &L, bool eloss, bool track, cudaStream_t s);
