@@ -345,7 +345,7 @@ def test_every_wire_fired_at_the_corners_of_step_and_window(field_kind, h, windo
     sc.close()
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_candidate_pool_overflow_is_recovered_by_a_second_pass(setup, variant):
     """More near-ties than the candidate pool holds: a plateau grid -- step = 0 on four
     axes, 16^5 = 1,048,576 nodes of which only 16 are distinct, each 65,536 times -- fills the 65,536-entry pool in
