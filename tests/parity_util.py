@@ -91,7 +91,7 @@ def explain_mismatch(bound, ev, seed, cfg, geom, dn=None, dchi2=None, same_track
     return bool(edge_window.any() or edge_zw.any() or at_exit.any() or at_R0.any())
 
 
-def compare_scan(cfg, geom, field, ev, grid, gpu, orc, sel, offset=0):
+def compare_scan(cfg, geom, field, ev, grid, gpu, orc, sel, offset=0, budget=True):
     """gpu: dict of concatenated per-seed arrays (+debug); orc: oracle.scan output on linear indices `sel`.
     Returns the list of exception seeds (each verified to be a threshold case)."""
     dbg = gpu["debug"][offset + sel]
@@ -113,7 +113,8 @@ def compare_scan(cfg, geom, field, ev, grid, gpu, orc, sel, offset=0):
                                 gpu_steps=int(dbg["n_steps"][i]), gpu_m_gas=int(dbg["m_gas"][i])), \
             f"seed {int(sel[i])}: n_match {nm_g[i]} vs {orc['n_match'][i]}, steps {dbg['n_steps'][i]} vs " \
             f"{orc['n_steps'][i]} without a threshold case within {EDGE_TOL_MM} mm"
-    assert len(bad) <= max(2, int(2e-3 * sel.size)), f"{len(bad)} threshold exceptions out of {sel.size}"
+    # (budget=False: the caller applies the 0.2 % budget to a whole campaign instead of to one small grid)
+    assert not budget or len(bad) <= max(2, int(2e-3 * sel.size)), f"{len(bad)} threshold exceptions out of {sel.size}"
     ok = np.ones(sel.size, dtype=bool); ok[bad] = False
     # chi2: fp32 accumulation of (D - drift)^2 with D good to ~2e-4 mm: |d chi2| <= n_match * 2 |d| dD
     assert np.all(np.abs(c2_g[ok] - orc["chi2"][ok]) <= 1e-3 * np.maximum(orc["n_match"][ok], 1))
