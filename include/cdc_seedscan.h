@@ -163,6 +163,24 @@ int32_t cdc_hough_seed_ranges(const cdc_geometry *g, const cdc_events *ev, const
                               int32_t charge, const float *d_zref_mm, double *d_ranges, int32_t *d_peak,
                               uint32_t *d_accum_or_null, void *stream);
 
+/* A2 without any allocation: the same Hough vote (same kernels, same results bit for bit) for callers that cannot
+ * allocate -- code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  It calls no
+ * cudaMalloc / cudaFree or allocating library routine, and needs no cdc_events handle (whose creation allocates): the
+ * hits are plain device arrays, d_hit_offsets [n_events + 1] (ascending, hits of event e are [offsets[e], offsets[e + 1]))
+ * and d_wire_id [offsets[n_events]], every id in [0, W) -- NOT checked here, an id outside reads outside the wire
+ * table.  g: a geometry created earlier (at set-up) on the current device.  Outputs as cdc_hough_seed_ranges (device,
+ * caller-owned; every element of d_accum_or_null is written).  The only scratch, one packed peak key per event, is a
+ * static device array of CDC_HOUGH_NOALLOC_MAX_EVENTS entries (32 KB on every GPU that loads the library, until exit):
+ * n_events beyond that is CDC_ERR_RANGE.  The first call on a device looks the array's address up (a call with
+ * n_events = 0 does only that and launches nothing: make it at set-up, before a capture).  EVERY call shares the array:
+ * each call clears the keys it uses on `stream` before the vote, but calls that overlap on the GPU (different streams,
+ * no ordering between them) race on it -- order them.  Asynchronous. */
+#define CDC_HOUGH_NOALLOC_MAX_EVENTS 4096
+int32_t cdc_hough_seed_ranges_noalloc(const cdc_geometry *g, int32_t n_events, const int32_t *d_hit_offsets,
+                                      const int32_t *d_wire_id, const cdc_hough_params *hp, int32_t charge,
+                                      const float *d_zref_mm, double *d_ranges, int32_t *d_peak,
+                                      uint32_t *d_accum_or_null, void *stream);
+
 /* A3-A7: the seed scan.  Every seed of every event's grid is propagated by Nystroem-RK4 (PAPER.md:55,
  * reading C5) in fp32 with compensated state, wires near each step are looked up (reading C8), owned
  * approaches to fired wires are scored (readings C9/C10), and the per-event maximum of

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(HERE, "libcdc_seedscan.so")
 
 EXPORTS = ["cdc_last_error", "cdc_geometry_create", "cdc_geometry_destroy", "cdc_geometry_wire_table",
            "cdc_event_upload", "cdc_events_destroy", "cdc_events_tables", "cdc_hough_dims",
-           "cdc_hough_seed_ranges", "cdc_seed_scan", "cdc_scan_get_stats", "cdc_best_track",
+           "cdc_hough_seed_ranges", "cdc_hough_seed_ranges_noalloc", "cdc_seed_scan", "cdc_scan_get_stats", "cdc_best_track",
            "cdc_find_tracks_host", "cdc_refine_tracks", "cdc_peel_turns", "cdc_classification_quality", "cdc_common_hits", "cdc_seed_scan_paper_mapping", "cdc_seed_scan_paper_mapping_v2", "cdc_seed_scan_adaptive", "cdc_fp32_peak_probe", "cdc_fp32_issue_probe", "cdc_kernel_launch_count"]
 
 
@@ -225,6 +225,17 @@ def cdc_hough_seed_ranges(geometry: Geometry, events: Events, hp: HoughParams, c
                           d_peak, d_accum=None, stream=None):
     _check(lib().cdc_hough_seed_ranges(geometry.handle, events.handle, C.byref(hp), C.c_int32(charge), _dp(d_zref),
                                        _dp(d_ranges), _dp(d_peak), _dp(d_accum), _stream(stream)))
+
+
+HOUGH_NOALLOC_MAX_EVENTS = 4096
+
+
+def cdc_hough_seed_ranges_noalloc(geometry: Geometry, n_events: int, d_hit_offsets, d_wire_id, hp: HoughParams, charge: int,
+                                  d_zref, d_ranges, d_peak, d_accum=None, stream=None):
+    """The Hough vote with its scratch in a static device array: no allocation, no Events handle (include/cdc_seedscan.h)."""
+    _check(lib().cdc_hough_seed_ranges_noalloc(geometry.handle, C.c_int32(n_events), _dp(d_hit_offsets), _dp(d_wire_id),
+                                               C.byref(hp), C.c_int32(charge), _dp(d_zref), _dp(d_ranges), _dp(d_peak),
+                                               _dp(d_accum), _stream(stream)))
 
 
 def cdc_seed_scan(geometry: Geometry, events: Events, grids: C.Array, params: ScanParams, d_best_key,

@@ -13,7 +13,7 @@ ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC,-ffp-contract=off,-Wall", *ARCH]
 SOURCES = {                      # file -> extra flags
     "abi.cu": [], "abi_events.cu": [], "abi_scan.cu": [], "abi_e2e.cu": [],
-    "events.cu": [], "hough.cu": [], "scan.cu": ["-Xptxas", "-v"], "scan_pair.cu": ["-Xptxas", "-v"], "scan_refill.cu": ["-Xptxas", "-v"], "scan_adaptive.cu": [], "peak.cu": [],
+    "events.cu": [], "hough.cu": [], "hough_noalloc.cu": [], "scan.cu": ["-Xptxas", "-v"], "scan_pair.cu": ["-Xptxas", "-v"], "scan_refill.cu": ["-Xptxas", "-v"], "scan_adaptive.cu": [], "peak.cu": [],
     "best.cu": ["-fmad=false"], "refine.cu": ["-fmad=false"], "abi_refine.cu": [], "quality.cu": [], "paper_v1.cu": [], "paper_v2.cu": [],
     "peel.cu": ["-fmad=false"], "abi_peel.cu": [],
 }
