@@ -327,11 +327,15 @@ void orc_seed_of_index(const double *lo, const double *step, const int32_t *nn, 
  * unchanged; the candidate wires are ALL hit wires (mode 0: the plain definition).
  * Outputs beyond orc_result: units (path in units of h), n_level[j] accepted steps per level (j < 8), and the decision
  * margins min |err - tol| / tol over rejections / acceptances and min |err - tol/32| / (tol/32) over the doubling
- * decisions (a GPU that takes its decisions in fp32 can differ where these are ~ 1e-5). */
+ * decisions (a GPU that takes its decisions in fp32 can differ where these are ~ 1e-5), and the same two distances
+ * in units of the stage derivatives, min |err - threshold| / H^2 (1/mm): the estimate is H^2 times a difference of
+ * four k, so the rounding noise of an fp32 evaluation is absolute in these units.  Diagnostics only: nothing of the
+ * propagation or of the decisions reads them. */
 typedef struct {
     int32_t units, n_level[8];
     double margin_tol, margin_up;
     uint32_t seq_hash;        /* hash of the accepted level sequence: hash = hash * 31 + (j + 1), mod 2^32 */
+    double kmargin_tol, kmargin_up;
 } orc_adaptive_info;
 
 void orc_eval_seed_adaptive(const orc_geom *g, const orc_field *f, const orc_hits *hits, const double *seed,
@@ -347,6 +351,7 @@ void orc_eval_seed_adaptive(const orc_geom *g, const orc_field *f, const orc_hit
     while (J < 7 && P->h * (double)(2 << J) <= h_max) ++J;      /* h 2^(J+1) <= h_max -> J + 1 */
     for (i = 0; i < 8; ++i) info->n_level[i] = 0;
     info->margin_tol = 1e300; info->margin_up = 1e300; info->seq_hash = 0u;
+    info->kmargin_tol = 1e300; info->kmargin_up = 1e300;
     r[0] = g->R0 * cos(seed[0]); r[1] = g->R0 * sin(seed[0]); r[2] = seed[1];
     p0 = sqrt(seed[2] * seed[2] + seed[3] * seed[3] + seed[4] * seed[4]);
     T[0] = seed[2] / p0; T[1] = seed[3] / p0; T[2] = seed[4] / p0;
@@ -360,6 +365,7 @@ void orc_eval_seed_adaptive(const orc_geom *g, const orc_field *f, const orc_hit
             orc_rkn_step_err(f, a, hj, r, T, rn, Tn, &err);
             mt = fabs(err - tol) / tol;
             if (mt < info->margin_tol) info->margin_tol = mt;
+            if (fabs(err - tol) / (hj * hj) < info->kmargin_tol) info->kmargin_tol = fabs(err - tol) / (hj * hj);
             if (err > tol && j > 0) { --j; continue; }
             break;
         }
@@ -403,6 +409,7 @@ void orc_eval_seed_adaptive(const orc_geom *g, const orc_field *f, const orc_hit
         if (j < J) {
             double mu = fabs(err - tol / 32.0) / (tol / 32.0);
             if (mu < info->margin_up) info->margin_up = mu;
+            if (fabs(err - tol / 32.0) / (hj * hj) < info->kmargin_up) info->kmargin_up = fabs(err - tol / 32.0) / (hj * hj);
             if (err <= tol / 32.0) ++j;
         }
     }
@@ -417,7 +424,7 @@ void orc_scan_adaptive(const orc_geom *g, const orc_field *f, const orc_hits *hi
                        const double *lo, const double *step, const int32_t *nn, const int64_t *index_list,
                        int64_t begin, int64_t end, const orc_params *P, double tol, double h_max,
                        int32_t *n_match, double *chi2, int32_t *n_steps, int32_t *units, int32_t *m_gas, double *final_r,
-                       int32_t *n_level /* [..][8] */, double *margins /* [..][2] */, uint32_t *seq_hash)
+                       int32_t *n_level /* [..][8] */, double *margins /* [..][4] */, uint32_t *seq_hash)
 {
     int64_t s;
     int i;
@@ -432,7 +439,8 @@ void orc_scan_adaptive(const orc_geom *g, const orc_field *f, const orc_hits *hi
         n_match[o] = res.n_match; chi2[o] = res.chi2; n_steps[o] = res.n_steps; units[o] = info.units; m_gas[o] = res.m_gas;
         final_r[3 * o] = res.r[0]; final_r[3 * o + 1] = res.r[1]; final_r[3 * o + 2] = res.r[2];
         for (i = 0; i < 8; ++i) n_level[8 * o + i] = info.n_level[i];
-        margins[2 * o] = info.margin_tol; margins[2 * o + 1] = info.margin_up; seq_hash[o] = info.seq_hash;
+        margins[4 * o] = info.margin_tol; margins[4 * o + 1] = info.margin_up; seq_hash[o] = info.seq_hash;
+        margins[4 * o + 2] = info.kmargin_tol; margins[4 * o + 3] = info.kmargin_up;
     }
 }
 

@@ -6,7 +6,9 @@ Draws small workloads at random -- config 0..4, event index, noise occupancy, dr
 shape (<= 6000 seeds), grid width, a grid shifted off the truth, kernel variant 0 / 1 / 2 -- scans each on the GPU through
 the C ABI and compares EVERY seed with the oracle exactly as the parity tests do (tests/parity_util.py: positions within
 1e-3 mm, identical step / in-gas / turn counts and n_match up to individually verified threshold cases, chi2 within its
-fp32 bound; best seed, its chi2 and the labels bit-exact against the oracle's arg max over the whole grid).  The 0.2 %
+fp32 bound; best seed, its chi2 and the labels bit-exact against the oracle's arg max over the whole grid).  Every
+fourth case also checks the Hough vote (accumulator, peak, ranges; parity_util.check_hough), every sixth the
+adaptive-step scan against the adaptive oracle (parity_util.compare_scan_adaptive).  The 0.2 %
 budget for threshold exceptions is applied to the campaign as a whole (with energy loss the seeds that share a start
 vertex within 1e-3 mm of R0 flip together, several on a grid of a thousand).  Prints one JSON summary line; a failed
 case is printed with what is needed to repeat it.  Exit status 1 on any failure."""
@@ -33,6 +35,7 @@ def main():
     fields = {0: synth.make_uniform_field(), 1: synth.make_table_field()}
     scanners = {k: api.SeedScanner(geom, f) for k, f in fields.items()}
     t0 = time.time(); n_cases = n_seeds = n_listed = n_skipped = 0; fails = []
+    n_hough = n_hough_bins = n_ad_cmp = n_ad_exc = n_ad_edge = 0
     while time.time() - t0 < budget_s:
         cfg = synth.CONFIGS[int(rng.integers(0, 5))]
         kw = {}
@@ -67,13 +70,25 @@ def main():
             n_listed += len(U.compare_scan(cfg, geom, field, ev, grid, gpu, orc, np.arange(grid.n_seeds), budget=False))
             U.check_best(cfg, geom, field, ev, grid, gpu, orc_full=orc)
             n_seeds += grid.n_seeds
+            if n_cases % 4 == 0:                  # A2: the Hough vote of this event against the oracle's
+                zref = float(ev.seed[1] + rng.uniform(-20.0, 20.0))
+                n_hough_bins += U.check_hough(geom, field, cfg, ev, zref, sc.hough(E, [zref], want_accum=True)); n_hough += 1
+            if n_cases % 6 == 1 and cfg.h_mm == 2.0 and grid.n_seeds <= 2500:      # 8(f) #4: the adaptive-step scan
+                tol, h_max = float(rng.choice([1e-4, 1e-5, 1e-6])), float(rng.choice([4.0, 8.0]))
+                desc["adaptive"] = dict(tol=tol, h_max=h_max)
+                ad = sc.scan_adaptive(sc.upload(*synth.pack_hits([ev])), [grid], U.gpu_params(cfg), tol, h_max)
+                exc, cmp_, edge = U.compare_scan_adaptive(cfg, geom, field, ev, grid, ad, 0, 0, tol, h_max)
+                n_ad_exc += exc; n_ad_cmp += cmp_; n_ad_edge += edge
         except Exception:
             fails.append(desc)
             print("FAIL", json.dumps(desc)); print(traceback.format_exc()[-1500:], flush=True)
         n_cases += 1
-    ok = not fails and n_listed <= 2e-3 * max(n_seeds, 1)
+    ok = (not fails and n_listed <= 2e-3 * max(n_seeds, 1) and n_ad_exc <= 0.05 * max(n_ad_exc + n_ad_cmp, 1)
+          and n_ad_edge <= max(2, 2e-3 * n_ad_cmp))
     print(json.dumps(dict(cases=n_cases, seeds=n_seeds, listed_threshold_exceptions=n_listed, failed_cases=len(fails),
-                          skipped_generator=n_skipped, seconds=round(time.time() - t0, 1), ok=ok)))
+                          hough_events=n_hough, hough_bins_differing_on_edge_votes=n_hough_bins,
+                          adaptive_seeds_same_step_sequence=n_ad_cmp, adaptive_decision_exceptions=n_ad_exc,
+                          adaptive_window_exceptions=n_ad_edge, skipped_generator=n_skipped, seconds=round(time.time() - t0, 1), ok=ok)))
     return 0 if ok else 1
 
 

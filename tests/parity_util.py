@@ -9,6 +9,8 @@ Tolerances (BASELINE.json north_star):
     or of a vertex where the in-gas flag changes) -- each such seed is listed and counted;
   * best seed and hit -> turn labels bit-exact (n_match and chi2 of the best seed bit-equal as doubles).
 """
+import math
+
 import numpy as np
 
 import oracle
@@ -147,3 +149,87 @@ def check_best(cfg, geom, field, ev, grid, gpu, e=0, hit_slice=None, orc_full=No
     got = gpu["labels"] if hit_slice is None else gpu["labels"][hit_slice]
     assert np.array_equal(got, lab), "hit -> turn labels differ"
     return b
+
+
+def hough_edge_votes(geom, ev, zref, hp, bins):
+    """Number of (hit, bin) pairs whose vote is within EDGE_TOL of the tolerance edge, for the listed bins."""
+    w = geom.wire[ev.wire_id].astype(np.float64)
+    t = zref / w[:, 4]
+    x, y = w[:, 0] + t * w[:, 2], w[:, 1] + t * w[:, 3]
+    n = 0
+    for (iR, icy, icx) in bins:
+        R = hp["R_lo_mm"] + (iR + 0.5) * hp["bin_R_mm"]
+        cy = -hp["half_xy_mm"] + (icy + 0.5) * hp["bin_xy_mm"]
+        cx = -hp["half_xy_mm"] + (icx + 0.5) * hp["bin_xy_mm"]
+        d = np.hypot(cx - x, cy - y)
+        edge = np.abs(np.abs(d - R) - hp["tol_mm"]) < EDGE_TOL_MM
+        elig = abs(math.hypot(cx, cy) - R) - (hp["origin_mm"] + hp["tol_mm"])
+        n += int(edge.sum()) + int(abs(elig) < EDGE_TOL_MM)
+    return n
+
+
+def check_hough(geom, field, cfg, ev, zref, h, e=0, max_diff=400):
+    """A2 of one event against the oracle: the accumulator bin for bin up to votes on the tolerance edge (every differing
+    bin must hold such a vote, and differ by at most 2), and -- when the oracle's peak is clear of the runner-up by more
+    than that, or nothing differs -- the same peak bin and the same (theta, px, py) ranges.  h: SeedScanner.hough(...,
+    want_accum=True).  Returns the number of differing bins."""
+    bound = oracle.Bound(geom, field, oracle_params(cfg))
+    z32 = float(np.float32(zref))
+    ho = oracle.hough(bound, ev.wire_id, ev.drift_mm, zref=z32)
+    acc_g, acc_o = h["accum"][e], ho["accum"]
+    diff = np.argwhere(acc_g != acc_o)
+    assert diff.shape[0] < max_diff, f"{diff.shape[0]} accumulator bins differ"
+    if diff.shape[0]:
+        assert hough_edge_votes(geom, ev, z32, B.HOUGH_DEFAULT, [tuple(x) for x in diff]) >= diff.shape[0]
+        assert np.abs(acc_g.astype(np.int64) - acc_o.astype(np.int64)).max() <= 2
+    runner_up = np.sort(acc_o.ravel())[-2]
+    if ho["peak"][3] - runner_up > 2 or diff.shape[0] == 0:
+        assert np.array_equal(h["peak"][e], ho["peak"])
+        assert np.allclose(h["ranges"][e], ho["ranges"], rtol=0, atol=1e-9)
+    return int(diff.shape[0])
+
+
+DECISION_EPS = 0.03
+# The estimate is H^2 max|k1 - k2 - k3 + k4|: its fp32 rounding noise is ABSOLUTE in units of k (|k| <= |a| B ~ 2.9e-3 / mm
+# at 105 MeV/c and 1 T, ulp32 = 2.3e-10), a few ulp, whatever the threshold.  At tol <= 1e-6 that exceeds 3 % of tol / 32.
+DECISION_K_EPS = 6e-10
+
+
+def _explain_adaptive(bound, ev, seed, cfg, geom, tol, h_max):
+    r = oracle.eval_seed_adaptive(bound, ev.wire_id, ev.drift_mm, seed, tol, h_max, records=True, rec_slack=0.1)
+    rec = r["rec"]
+    return bool((np.abs(np.abs(rec["resid"]) - cfg.window_mm) < EDGE_TOL_MM).any() or
+                (np.abs(np.abs(rec["zw"]) - geom.z_half_mm) < EDGE_TOL_MM).any())
+
+
+def compare_scan_adaptive(cfg, geom, field, ev, grid, gpu, o, e, tol, h_max):
+    """Event e (seeds [o, o + n_seeds) of the concatenated outputs) of SeedScanner.scan_adaptive against the adaptive
+    oracle, by the protocol in the header of test_gpu_adaptive.py.  Returns (decision-threshold exceptions, seeds compared,
+    window / wire-end exceptions)."""
+    ns = grid.n_seeds
+    orc = oracle.scan_adaptive_parallel(geom, field, oracle_params(cfg), ev.wire_id, ev.drift_mm, grid, tol, h_max)
+    dbg = gpu["debug"][o:o + ns]
+    exc = ((orc["margins"][:, 0] < DECISION_EPS) | (orc["margins"][:, 1] < DECISION_EPS) |         # (a)
+           (orc["margins"][:, 2] < DECISION_K_EPS) | (orc["margins"][:, 3] < DECISION_K_EPS))
+    ok = ~exc
+    # (b) identical step-length sequence
+    assert np.array_equal(gpu["seq_hash"][o:o + ns][ok], orc["seq_hash"][ok])
+    assert np.array_equal(dbg["n_steps"][ok], orc["n_steps"][ok]) and np.array_equal(dbg["pad"][ok], orc["units"][ok])
+    assert np.array_equal(gpu["n_level"][o:o + ns][ok], orc["n_level"][ok][:, :7])
+    # (c) positions, in-gas units, match counts
+    pos = np.stack([dbg["x"], dbg["y"], dbg["z"]], axis=1)
+    if ok.any():
+        assert np.linalg.norm(pos - orc["final_r"], axis=1)[ok].max() < POS_TOL_MM
+    assert np.array_equal(dbg["m_gas"][ok], orc["m_gas"][ok])
+    nm_g = gpu["n_match"][o:o + ns]; c2_g = gpu["chi2"][o:o + ns]
+    bad = np.flatnonzero(ok & (nm_g != orc["n_match"]))
+    bound = oracle.Bound(geom, field, oracle_params(cfg))
+    for i in bad:
+        assert _explain_adaptive(bound, ev, grid.node(grid.unravel(int(i))), cfg, geom, tol, h_max), \
+            f"seed {i}: n_match {nm_g[i]} vs {orc['n_match'][i]} without a threshold case"
+    good = ok.copy(); good[bad] = False
+    assert np.all(np.abs(c2_g[good] - orc["chi2"][good]) <= 1e-3 * np.maximum(orc["n_match"][good], 1))
+    # the fused fp32 arg max is the arg max of the per-seed fp32 scores
+    S32 = nm_g.astype(np.float32) - c2_g / np.float32(cfg.window_mm ** 2)
+    assert abs(float(gpu["S32_max"][e]) - float(np.maximum(S32, 0).max())) < 1e-5
+    return int(exc.sum()), int(ok.sum()), int(bad.size)

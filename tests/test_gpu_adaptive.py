@@ -4,7 +4,9 @@ oracle's adaptive-step evaluation (oracle/cdc_oracle.c orc_eval_seed_adaptive), 
 Parity protocol of this variant.  The step-size decisions are taken in fp32 by the kernel and in
 fp64 by the oracle, and a different decision changes every later vertex, so:
   (a) a seed whose oracle-side error estimate comes within DECISION_EPS (relative) of tol, or of tol / 32, at any
-      decision is an explicit EXCEPTION CLASS: listed and counted, not compared further;
+      decision -- or within DECISION_K_EPS H^2 of it: the fp32 rounding noise of the estimate, a few ulp of the stage
+      derivatives, which is the larger of the two at tol <= 1e-6 -- is an explicit EXCEPTION CLASS: listed and counted,
+      not compared further (parity_util.compare_scan_adaptive);
   (b) every other seed must take the IDENTICAL sequence of step lengths (equal hash of the level sequence, equal number
       of steps, path units and steps per level), and then
   (c) final positions agree within 1e-3 mm, in-gas units are equal, and n_match is identical except the usual listed
@@ -20,16 +22,6 @@ import parity_util as U
 
 pytestmark = pytest.mark.gpu
 
-DECISION_EPS = 0.03
-
-
-def _explain_adaptive(bound, ev, seed, cfg, geom, tol, h_max):
-    r = oracle.eval_seed_adaptive(bound, ev.wire_id, ev.drift_mm, seed, tol, h_max, records=True, rec_slack=0.1)
-    rec = r["rec"]
-    return bool((np.abs(np.abs(rec["resid"]) - cfg.window_mm) < U.EDGE_TOL_MM).any() or
-                (np.abs(np.abs(rec["zw"]) - geom.z_half_mm) < U.EDGE_TOL_MM).any())
-
-
 @pytest.mark.parametrize("cfg_id,grid_n,tol,h_max", [(1, 6, 1e-5, 8.0), (3, 6, 1e-5, 8.0), (3, 5, 1e-4, 8.0), (3, 5, 3e-7, 4.0),
                                                      (2, 5, 1e-5, 8.0)])
 def test_adaptive_scan_against_the_adaptive_oracle(cfg_id, grid_n, tol, h_max):
@@ -42,31 +34,8 @@ def test_adaptive_scan_against_the_adaptive_oracle(cfg_id, grid_n, tol, h_max):
     o = 0
     for e, (ev, grid) in enumerate(zip(events, grids)):
         ns = grid.n_seeds
-        orc = oracle.scan_adaptive_parallel(geom, field, U.oracle_params(cfg), ev.wire_id, ev.drift_mm, grid, tol, h_max)
-        dbg = gpu["debug"][o:o + ns]
-        exc = (orc["margins"][:, 0] < DECISION_EPS) | (orc["margins"][:, 1] < DECISION_EPS)           # (a)
-        ok = ~exc
-        n_exc += int(exc.sum()); n_cmp += int(ok.sum())
-        # (b) identical step-length sequence
-        assert np.array_equal(gpu["seq_hash"][o:o + ns][ok], orc["seq_hash"][ok])
-        assert np.array_equal(dbg["n_steps"][ok], orc["n_steps"][ok]) and np.array_equal(dbg["pad"][ok], orc["units"][ok])
-        assert np.array_equal(gpu["n_level"][o:o + ns][ok], orc["n_level"][ok][:, :7])
-        # (c) positions, in-gas units, match counts
-        pos = np.stack([dbg["x"], dbg["y"], dbg["z"]], axis=1)
-        assert np.linalg.norm(pos - orc["final_r"], axis=1)[ok].max() < U.POS_TOL_MM
-        assert np.array_equal(dbg["m_gas"][ok], orc["m_gas"][ok])
-        nm_g = gpu["n_match"][o:o + ns]; c2_g = gpu["chi2"][o:o + ns]
-        bad = np.flatnonzero(ok & (nm_g != orc["n_match"]))
-        bound = oracle.Bound(geom, field, U.oracle_params(cfg))
-        for i in bad:
-            assert _explain_adaptive(bound, ev, grid.node(grid.unravel(int(i))), cfg, geom, tol, h_max), \
-                f"seed {i}: n_match {nm_g[i]} vs {orc['n_match'][i]} without a threshold case"
-        n_edge += bad.size
-        good = ok.copy(); good[bad] = False
-        assert np.all(np.abs(c2_g[good] - orc["chi2"][good]) <= 1e-3 * np.maximum(orc["n_match"][good], 1))
-        # the fused fp32 arg max is the arg max of the per-seed fp32 scores
-        S32 = nm_g.astype(np.float32) - c2_g / np.float32(cfg.window_mm ** 2)
-        assert abs(float(gpu["S32_max"][e]) - float(np.maximum(S32, 0).max())) < 1e-5
+        exc, cmp_, edge = U.compare_scan_adaptive(cfg, geom, field, ev, grid, gpu, o, e, tol, h_max)
+        n_exc += exc; n_cmp += cmp_; n_edge += edge
         o += ns
     assert n_exc <= 0.05 * (n_exc + n_cmp) and n_edge <= max(2, int(2e-3 * n_cmp))
     assert int(gpu["n_level"][:, 1:].sum()) > 0 or tol < 1e-6            # longer steps were actually taken

@@ -126,23 +126,6 @@ def test_cfg1_full_size_every_seed(torch_cuda):
 
 
 # ------------------------------------------------------------------ config 2: Hough ranges, energy loss, 24^5
-def _hough_edge_votes(geom, ev, zref, hp, bins):
-    """Number of (hit, bin) pairs whose vote is within EDGE_TOL of the tolerance edge, for the listed bins."""
-    w = geom.wire[ev.wire_id].astype(np.float64)
-    t = zref / w[:, 4]
-    x, y = w[:, 0] + t * w[:, 2], w[:, 1] + t * w[:, 3]
-    n = 0
-    for (iR, icy, icx) in bins:
-        R = hp["R_lo_mm"] + (iR + 0.5) * hp["bin_R_mm"]
-        cy = -hp["half_xy_mm"] + (icy + 0.5) * hp["bin_xy_mm"]
-        cx = -hp["half_xy_mm"] + (icx + 0.5) * hp["bin_xy_mm"]
-        d = np.hypot(cx - x, cy - y)
-        edge = np.abs(np.abs(d - R) - hp["tol_mm"]) < U.EDGE_TOL_MM
-        elig = abs(math.hypot(cx, cy) - R) - (hp["origin_mm"] + hp["tol_mm"])
-        n += int(edge.sum()) + int(abs(elig) < U.EDGE_TOL_MM)
-    return n
-
-
 @pytest.mark.parametrize("n_events", [1, 3, 6])
 def test_hough_accumulator_is_independent_of_the_batch_size(torch_cuda, n_events):
     """The accumulator of an event does not depend on what else is in the batch (one grid row per event), and the
@@ -164,7 +147,7 @@ def test_hough_accumulator_is_independent_of_the_batch_size(torch_cuda, n_events
         diff = np.argwhere(h["accum"][e] != ho["accum"])
         assert diff.shape[0] < 400
         if diff.shape[0]:
-            assert _hough_edge_votes(geom, events[e], float(np.float32(zref[e])), B.HOUGH_DEFAULT,
+            assert U.hough_edge_votes(geom, events[e], float(np.float32(zref[e])), B.HOUGH_DEFAULT,
                                      [tuple(x) for x in diff]) >= diff.shape[0]
     sc.close(); one.close()
 
@@ -185,7 +168,7 @@ def test_cfg2_hough_ranges_eloss_full_size(torch_cuda):
     diff = np.argwhere(acc_g != acc_o)
     assert diff.shape[0] < 200
     if diff.shape[0]:
-        n_edge = _hough_edge_votes(geom, ev, float(np.float32(zref)), B.HOUGH_DEFAULT, [tuple(x) for x in diff])
+        n_edge = U.hough_edge_votes(geom, ev, float(np.float32(zref)), B.HOUGH_DEFAULT, [tuple(x) for x in diff])
         assert n_edge >= diff.shape[0]                      # every differing bin has an edge vote
         assert np.abs(acc_g.astype(np.int64) - acc_o.astype(np.int64)).max() <= 2
     runner_up = np.sort(acc_o.ravel())[-2]
