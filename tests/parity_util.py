@@ -211,7 +211,10 @@ def compare_scan_adaptive(cfg, geom, field, ev, grid, gpu, o, e, tol, h_max):
     dbg = gpu["debug"][o:o + ns]
     exc = ((orc["margins"][:, 0] < DECISION_EPS) | (orc["margins"][:, 1] < DECISION_EPS) |         # (a)
            (orc["margins"][:, 2] < DECISION_K_EPS) | (orc["margins"][:, 3] < DECISION_K_EPS))
-    ok = ~exc
+    # a vertex within 1e-3 mm of R0 (the fixed-step protocol's listed class, SURVEY 8(d) parity procedure (ii)): its in-gas
+    # flag is a threshold decision; where the in-gas units differ AND the oracle saw such a vertex, the seed is listed
+    r0x = ~exc & (dbg["m_gas"] != orc["m_gas"]) & (orc["margins"][:, 4] < EDGE_TOL_MM)
+    ok = ~exc & ~r0x
     # (b) identical step-length sequence
     assert np.array_equal(gpu["seq_hash"][o:o + ns][ok], orc["seq_hash"][ok])
     assert np.array_equal(dbg["n_steps"][ok], orc["n_steps"][ok]) and np.array_equal(dbg["pad"][ok], orc["units"][ok])
@@ -232,4 +235,4 @@ def compare_scan_adaptive(cfg, geom, field, ev, grid, gpu, o, e, tol, h_max):
     # the fused fp32 arg max is the arg max of the per-seed fp32 scores
     S32 = nm_g.astype(np.float32) - c2_g / np.float32(cfg.window_mm ** 2)
     assert abs(float(gpu["S32_max"][e]) - float(np.maximum(S32, 0).max())) < 1e-5
-    return int(exc.sum()), int(ok.sum()), int(bad.size)
+    return int(exc.sum()), int(ok.sum()), int(bad.size) + int(r0x.sum())
