@@ -256,7 +256,7 @@ def bin_event(bound: Bound, wire_id, drift) -> np.ndarray:
 class OrcAdaptiveInfo(C.Structure):
     _fields_ = [("units", C.c_int32), ("n_level", C.c_int32 * 8), ("margin_tol", C.c_double), ("margin_up", C.c_double),
                 ("seq_hash", C.c_uint32), ("kmargin_tol", C.c_double), ("kmargin_up", C.c_double),
-                ("r0_margin", C.c_double)]
+                ("r0_margin", C.c_double), ("exit_margin", C.c_double)]
 
 
 def eval_seed_adaptive(bound: Bound, wire_id, drift, seed, tol: float, h_max: float, records: bool = False,
@@ -274,7 +274,8 @@ def eval_seed_adaptive(bound: Bound, wire_id, drift, seed, tol: float, h_max: fl
     out = dict(n_match=res.n_match, chi2=res.chi2, n_steps=res.n_steps, turns=res.turns, m_gas=res.m_gas,
                r=np.array(res.r[:]), T=np.array(res.T[:]), p=res.p, units=info.units, n_level=np.array(info.n_level[:]),
                margin_tol=info.margin_tol, margin_up=info.margin_up, seq_hash=int(info.seq_hash),
-               kmargin_tol=info.kmargin_tol, kmargin_up=info.kmargin_up, r0_margin=info.r0_margin)
+               kmargin_tol=info.kmargin_tol, kmargin_up=info.kmargin_up, r0_margin=info.r0_margin,
+               exit_margin=info.exit_margin)
     if records:
         out["rec"] = rec[:res.n_rec]
     return out
@@ -290,7 +291,7 @@ def scan_adaptive(bound: Bound, wire_id, drift, grid, tol: float, h_max: float, 
         end = int(il.size) if il is not None else int(np.prod(nn.astype(np.int64)))
     n = end - begin
     nm = np.zeros(n, dtype=np.int32); c2 = np.zeros(n); ns = np.zeros(n, dtype=np.int32); un = np.zeros(n, dtype=np.int32)
-    mg = np.zeros(n, dtype=np.int32); fr = np.zeros((n, 3)); nl = np.zeros((n, 8), dtype=np.int32); mar = np.zeros((n, 5))
+    mg = np.zeros(n, dtype=np.int32); fr = np.zeros((n, 3)); nl = np.zeros((n, 8), dtype=np.int32); mar = np.zeros((n, 6))
     sh = np.zeros(n, dtype=np.uint32)
     lib().orc_scan_adaptive(C.byref(bound.g), C.byref(bound.f), C.byref(H), _p(lo), _p(st), _p(nn), _p(il),
                             C.c_int64(begin), C.c_int64(end), C.byref(bound.P), C.c_double(tol), C.c_double(h_max),

@@ -338,6 +338,8 @@ typedef struct {
     double kmargin_tol, kmargin_up;
     double r0_margin;         /* min | |r_n|_xy - R0 | over the vertices n >= 1 (mm): the in-gas flag of a vertex this close to
                                * R0 is a threshold decision (diagnostic, like the margins) */
+    double exit_margin;       /* min over the vertices n >= 1 of min(| |z_n| - z_half |, | |r_n|_xy - r_out |) (mm): likewise
+                               * for the termination tests */
 } orc_adaptive_info;
 
 void orc_eval_seed_adaptive(const orc_geom *g, const orc_field *f, const orc_hits *hits, const double *seed,
@@ -353,7 +355,7 @@ void orc_eval_seed_adaptive(const orc_geom *g, const orc_field *f, const orc_hit
     while (J < 7 && P->h * (double)(2 << J) <= h_max) ++J;      /* h 2^(J+1) <= h_max -> J + 1 */
     for (i = 0; i < 8; ++i) info->n_level[i] = 0;
     info->margin_tol = 1e300; info->margin_up = 1e300; info->seq_hash = 0u;
-    info->kmargin_tol = 1e300; info->kmargin_up = 1e300; info->r0_margin = 1e300;
+    info->kmargin_tol = 1e300; info->kmargin_up = 1e300; info->r0_margin = 1e300; info->exit_margin = 1e300;
     r[0] = g->R0 * cos(seed[0]); r[1] = g->R0 * sin(seed[0]); r[2] = seed[1];
     p0 = sqrt(seed[2] * seed[2] + seed[3] * seed[3] + seed[4] * seed[4]);
     T[0] = seed[2] / p0; T[1] = seed[3] / p0; T[2] = seed[4] / p0;
@@ -403,6 +405,9 @@ void orc_eval_seed_adaptive(const orc_geom *g, const orc_field *f, const orc_hit
         c_next = (r[0] * r[0] + r[1] * r[1] >= g->R0 * g->R0);
         if (fabs(sqrt(r[0] * r[0] + r[1] * r[1]) - g->R0) < info->r0_margin)
             info->r0_margin = fabs(sqrt(r[0] * r[0] + r[1] * r[1]) - g->R0);
+        if (fabs(fabs(r[2]) - g->z_half) < info->exit_margin) info->exit_margin = fabs(fabs(r[2]) - g->z_half);
+        if (fabs(sqrt(r[0] * r[0] + r[1] * r[1]) - g->r_out) < info->exit_margin)
+            info->exit_margin = fabs(sqrt(r[0] * r[0] + r[1] * r[1]) - g->r_out);
         if (!c_n && c_next) t += 1;
         c_n = c_next;
         if (fabs(r[2]) > g->z_half) break;
@@ -428,7 +433,7 @@ void orc_scan_adaptive(const orc_geom *g, const orc_field *f, const orc_hits *hi
                        const double *lo, const double *step, const int32_t *nn, const int64_t *index_list,
                        int64_t begin, int64_t end, const orc_params *P, double tol, double h_max,
                        int32_t *n_match, double *chi2, int32_t *n_steps, int32_t *units, int32_t *m_gas, double *final_r,
-                       int32_t *n_level /* [..][8] */, double *margins /* [..][5] */, uint32_t *seq_hash)
+                       int32_t *n_level /* [..][8] */, double *margins /* [..][6] */, uint32_t *seq_hash)
 {
     int64_t s;
     int i;
@@ -443,8 +448,9 @@ void orc_scan_adaptive(const orc_geom *g, const orc_field *f, const orc_hits *hi
         n_match[o] = res.n_match; chi2[o] = res.chi2; n_steps[o] = res.n_steps; units[o] = info.units; m_gas[o] = res.m_gas;
         final_r[3 * o] = res.r[0]; final_r[3 * o + 1] = res.r[1]; final_r[3 * o + 2] = res.r[2];
         for (i = 0; i < 8; ++i) n_level[8 * o + i] = info.n_level[i];
-        margins[5 * o] = info.margin_tol; margins[5 * o + 1] = info.margin_up; seq_hash[o] = info.seq_hash;
-        margins[5 * o + 2] = info.kmargin_tol; margins[5 * o + 3] = info.kmargin_up; margins[5 * o + 4] = info.r0_margin;
+        margins[6 * o] = info.margin_tol; margins[6 * o + 1] = info.margin_up; seq_hash[o] = info.seq_hash;
+        margins[6 * o + 2] = info.kmargin_tol; margins[6 * o + 3] = info.kmargin_up; margins[6 * o + 4] = info.r0_margin;
+        margins[6 * o + 5] = info.exit_margin;
     }
 }
 

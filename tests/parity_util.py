@@ -214,6 +214,8 @@ def compare_scan_adaptive(cfg, geom, field, ev, grid, gpu, o, e, tol, h_max):
     # a vertex within 1e-3 mm of R0 (the fixed-step protocol's listed class, SURVEY 8(d) parity procedure (ii)): its in-gas
     # flag is a threshold decision; where the in-gas units differ AND the oracle saw such a vertex, the seed is listed
     r0x = ~exc & (dbg["m_gas"] != orc["m_gas"]) & (orc["margins"][:, 4] < EDGE_TOL_MM)
+    # likewise a vertex within 1e-3 mm of |z| = z_half or of r_out: one side ends the track a step before the other
+    r0x |= ~exc & (dbg["n_steps"] != orc["n_steps"]) & (orc["margins"][:, 5] < EDGE_TOL_MM)
     ok = ~exc & ~r0x
     # (b) identical step-length sequence
     assert np.array_equal(gpu["seq_hash"][o:o + ns][ok], orc["seq_hash"][ok])

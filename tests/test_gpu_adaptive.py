@@ -7,7 +7,8 @@ fp64 by the oracle, and a different decision changes every later vertex, so:
       decision -- or within DECISION_K_EPS H^2 of it: the fp32 rounding noise of the estimate, a few ulp of the stage
       derivatives, which is the larger of the two at tol <= 1e-6 -- is an explicit EXCEPTION CLASS: listed and counted,
       not compared further (parity_util.compare_scan_adaptive); so is a seed whose in-gas units differ while one of
-      the oracle's vertices lies within 1e-3 mm of R0 (the in-gas flag of that vertex is a threshold decision);
+      the oracle's vertices lies within 1e-3 mm of R0 (the in-gas flag of that vertex is a threshold decision), or
+      whose step counts differ while one lies within 1e-3 mm of |z| = z_half or r_out (the exit tests);
   (b) every other seed must take the IDENTICAL sequence of step lengths (equal hash of the level sequence, equal number
       of steps, path units and steps per level), and then
   (c) final positions agree within 1e-3 mm, in-gas units are equal, and n_match is identical except the usual listed
