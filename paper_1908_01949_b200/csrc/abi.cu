@@ -193,6 +193,25 @@ extern "C" int32_t cdc_geometry_create(const cdc_geometry_desc *gd, const cdc_fi
                         make_float4((float)(0.25 * (n00 + n01 + n10 + n11)), (float)((n10 - n00) + 0.5 * crz),
                                     (float)((n01 - n00) + 0.5 * crz), (float)crz);
                 }
+        // bound of the Cartesian gradient of B = (B_r x / rho, B_r y / rho, B_z) over the table: within a bilinear cell a
+        // partial derivative lies between its values on the two opposite edges; the azimuthal term is B_r / rho
+        double gz[2] = {0, 0}, gr[2] = {0, 0}, gphi = 0;
+        for (int iz = 0; iz < fd->nz; ++iz)
+            for (int ir = 0; ir < fd->nr; ++ir)
+                for (int c = 0; c < 2; ++c) {
+                    const double v = g->field_tab[((size_t)iz * fd->nr + ir) * 2 + c];
+                    if (iz + 1 < fd->nz) gz[c] = std::max(gz[c], fabs(g->field_tab[((size_t)(iz + 1) * fd->nr + ir) * 2 + c] - v) / fd->dz_mm);
+                    if (ir + 1 < fd->nr) gr[c] = std::max(gr[c], fabs(g->field_tab[((size_t)iz * fd->nr + ir + 1) * 2 + c] - v) / fd->dr_mm);
+                    if (c == 0) {
+                        const double rho = fd->r0_mm + ir * fd->dr_mm;
+                        // |B_r| / rho on the cell [rho_i, rho_i+1]: node value over the inner radius; on the axis B_r
+                        // must vanish (then B_r / rho <= the radial slope, already in gr[0])
+                        if (rho > 0) gphi = std::max(gphi, fabs(v) / rho);
+                        else if (v != 0.0) gphi = INFINITY;
+                        if (ir > 0 && fd->r0_mm + (ir - 1) * fd->dr_mm > 0) gphi = std::max(gphi, fabs(v) / (fd->r0_mm + (ir - 1) * fd->dr_mm));
+                    }
+                }
+        g->grad_max = gz[0] + gz[1] + gr[0] + gr[1] + gphi;
         G_CUDA(dev_alloc(&g->d_cells, cells.size()));
         G_CUDA(cudaMemcpy(g->d_cells, cells.data(), sizeof(float4) * cells.size(), cudaMemcpyHostToDevice));
     }
@@ -208,6 +227,7 @@ extern "C" int32_t cdc_geometry_create(const cdc_geometry_desc *gd, const cdc_fi
     f.kind = fd->kind; f.bz = (float)fd->bz_T; f.nr = fd->nr; f.nz = fd->nz;
     f.r0 = (float)fd->r0_mm; f.z0 = (float)fd->z0_mm;
     f.inv_dr = fd->kind == 1 ? (float)(1.0 / fd->dr_mm) : 0.f; f.inv_dz = fd->kind == 1 ? (float)(1.0 / fd->dz_mm) : 0.f;
+    f.grad_max = (float)g->grad_max;
     f.tab = g->d_field; f.cells = g->d_cells; f.n_cells = fd->kind == 1 ? (fd->nr - 1) * (fd->nz - 1) : 0;
     f.cr = fd->kind == 1 ? (float)(-fd->r0_mm / fd->dr_mm - 0.5) : 0.f; f.cz = fd->kind == 1 ? (float)(-fd->z0_mm / fd->dz_mm - 0.5) : 0.f;
     Geom64 &q = g->g64;

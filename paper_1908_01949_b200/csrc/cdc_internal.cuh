@@ -34,6 +34,7 @@ struct FieldDev {
     float r0, z0, inv_dr, inv_dz;
     float cr, cz;            // -r0 / dr - 1/2, -z0 / dz - 1/2: fma(rho, inv_dr, cr) = cell coordinate - 1/2
     int32_t n_cells;         // (nr - 1) (nz - 1)
+    float grad_max;          // bound of |dB/dx| over the table (T/mm; +inf if B_r != 0 on the axis): see scan.cu, field reuse
     const float2 *tab;       // [nz][nr] (B_r, B_z) nodes (fp64 path)
     const float4 *cells;     // [nr-1][nz-1][2] (z fastest): bilinear coefficients about the cell centre (c0, c_z, c_r, c_rz) of B_r, then of B_z
 };
@@ -68,6 +69,7 @@ struct cdc_geometry {
     std::vector<float> wire5;
     double z_half = 0, R0 = 0, r_out = 0;
     double b_max = 0;                        // largest |B| of the field description
+    double grad_max = 0;                     // bound of the gradient of B over the table (T/mm), 0 for the uniform field
     double cell_max = 0;                     // largest cell width (arc at the end plate)
     double pitch = 0, excl = 0;              // layer pitch; distance below which a wire is surely in the 2 x 2 set
     float uz = 1.f;

@@ -28,6 +28,9 @@ struct ScanArgs {
     // around the seeds' own positions (tight curls, or K < 1): K0 = min(lookup_every_tight, 1 + floor((k_margin0 - sep) * inv_h))
     // (sep = half the two seeds' separation as a wire sees it; above sep_cap the pair does one lookup per seed)
     float k_margin, k_margin0, two_inv_h, inv_h, sin_eps, sep_cap;
+    // field reuse (tabulated field): B at a step's start vertex is taken from the previous step's 4th-stage point where
+    // reuse_c |a| (|a| reuse_b2 + grad_max) <= reuse_eps (scan.cu)
+    float reuse_c, reuse_b2, reuse_eps;
     float margin;
     uint32_t *n_match;
     float *chi2;
