@@ -30,6 +30,9 @@ METRIC = "seed_propagations_per_s"
 UNIT = "seeds/s"
 # Algorithmic FP32 flops (FMA = 2) of the scan kernel's arithmetic, DESIGN.md section 7
 FLOPS_STEP = {0: 78.0, 1: 237.0}        # per RKN step, uniform / tabulated field (compensated state included)
+# what the kernel executes for the same step: the closed-form map in the uniform field; in the tabulated field two table
+# look-ups per step instead of three (the start vertex's B is carried from the previous 4th stage: scan.cu, field reuse)
+FLOPS_STEP_EXECUTED = {0: 56.0, 1: 212.0}
 FLOPS_LOOKUP, FLOPS_G, FLOPS_APPROACH = 43.0, 22.0, 35.0
 PEAK_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # 74.4: 148 SMs x 128 FP32 lanes x 2 x 1965 MHz (B200_PROFILING.md)
 
@@ -345,8 +348,12 @@ def measure(args, workload, steps, warmup, rank, world, local, dist, with_cpu_ba
                          "kernel": "seed_scan_kernel",
                          "flops_per_rkn_step": flops / max(acc["n_steps"], 1),
                          "note": "flops = the step as the method defines it (DESIGN.md section 7)" +
-                                 ("" if cfg.field_kind else "; the uniform-field kernel executes its closed form, 56 "
-                                  "instead of 78 flops per step"),
+                                 ("; the tabulated-field kernel carries B at a step's start vertex over from the previous "
+                                  "step's 4th-stage point (within half an ulp32 of B): it executes 212 instead of 237 "
+                                  "flops per step" if cfg.field_kind else
+                                  "; the uniform-field kernel executes its closed form, 56 instead of 78 flops per step"),
+                         "frac_executed": (achieved - (FLOPS_STEP[cfg.field_kind] - FLOPS_STEP_EXECUTED[cfg.field_kind]) *
+                                           acc["n_steps"] / k_s / 1e12) / PEAK_FP32_TFLOPS,
                          "peak_source": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (nominal, B200_PROFILING.md; "
                                         "MEASURED_PEAKS.json has no FP32 figure)"}}
     f, _ = B.cdc_fp32_peak_probe(4096)

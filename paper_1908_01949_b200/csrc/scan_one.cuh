@@ -128,9 +128,10 @@ __device__ __forceinline__ void slot_step(const ScanArgs &A, const float *drift_
     g = gn;
 }
 
-// tabulated field at (x, y, z): field_at<1>() of scan_common.cuh with (B_x, B_y), the two cell coordinates and the two
-// halves of each bilinear form carried as packed pairs (same operations, same rounding)
-__device__ __forceinline__ void field_at_p(const FieldDev &F, f2 xy, float z, f2 &Bxy, float &Bz)
+// a B at (x, y, z), a = kappa q / p: the tabulated field of field_at<1>() (scan_common.cuh) with (B_x, B_y), the two cell
+// coordinates and the two halves of each bilinear form carried as packed pairs, and the seed's a folded in here (two
+// multiplies per evaluation) instead of into each component of each stage derivative (three per stage: k = U x (a B))
+__device__ __forceinline__ void field_at_p(const FieldDev &F, float a, f2 xy, float z, f2 &Bxy, float &Bz)
 {
     const float x = lo(xy), y = hi(xy);
     const float rho2 = fmaf(x, x, y * y);
@@ -146,8 +147,8 @@ __device__ __forceinline__ void field_at_p(const FieldDev &F, f2 xy, float z, f2
     const float4 cr = __ldg(c), cz = __ldg(c + 1);                                  // (c0, c_z, c_r, c_rz) of B_r, of B_z
     const f2 tr = fma2(bc(lo(w)), pk(cr.z, cr.w), pk(cr.x, cr.y)), tz = fma2(bc(lo(w)), pk(cz.z, cz.w), pk(cz.x, cz.y));
     const float Br = fmaf(hi(w), hi(tr), lo(tr));
-    Bz = fmaf(hi(w), hi(tz), lo(tz));
-    Bxy = mul2(bc(Br * inv_rho), xy);
+    Bz = a * fmaf(hi(w), hi(tz), lo(tz));
+    Bxy = mul2(bc((a * Br) * inv_rho), xy);
 }
 
 }  // namespace

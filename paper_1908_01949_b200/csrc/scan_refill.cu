@@ -221,27 +221,27 @@ __global__ void __launch_bounds__(kBlock, FIELD == 0 ? REFILL_MB0 : REFILL_MB1) 
             } else {
                 f2 Bxy;
                 float Bz;
-                if (n == 0 || !reuse) field_at_p(A.fd, xyh, zh, Bxy_c, Bz_c);     // else: carried from the last 4th stage
+                if (n == 0 || !reuse) field_at_p(A.fd, a, xyh, zh, Bxy_c, Bz_c);     // else: carried from the last 4th stage
                 Bxy = Bxy_c; Bz = Bz_c;
                 float Ux = lo(Txyh), Uy = hi(Txyh), Uz = Tzh;
-                const f2 k1xy = pk(a * fmaf(Uy, Bz, -Uz * hi(Bxy)), a * fmaf(Uz, lo(Bxy), -Ux * Bz));
-                const float k1z = a * fmaf(Ux, hi(Bxy), -Uy * lo(Bxy));
+                const f2 k1xy = pk(fmaf(Uy, Bz, -Uz * hi(Bxy)), fmaf(Uz, lo(Bxy), -Ux * Bz));
+                const float k1z = fmaf(Ux, hi(Bxy), -Uy * lo(Bxy));
                 f2 Uxy = fma2(bc(A.h_half), k1xy, Txyh);
                 Uz = fmaf(A.h_half, k1z, Tzh);
-                field_at_p(A.fd, fma2(bc(A.h2_8), k1xy, fma2(bc(A.h_half), Txyh, xyh)), fmaf(A.h2_8, k1z, fmaf(A.h_half, Tzh, zh)), Bxy, Bz);
+                field_at_p(A.fd, a, fma2(bc(A.h2_8), k1xy, fma2(bc(A.h_half), Txyh, xyh)), fmaf(A.h2_8, k1z, fmaf(A.h_half, Tzh, zh)), Bxy, Bz);
                 Ux = lo(Uxy); Uy = hi(Uxy);
-                const f2 k2xy = pk(a * fmaf(Uy, Bz, -Uz * hi(Bxy)), a * fmaf(Uz, lo(Bxy), -Ux * Bz));
-                const float k2z = a * fmaf(Ux, hi(Bxy), -Uy * lo(Bxy));
+                const f2 k2xy = pk(fmaf(Uy, Bz, -Uz * hi(Bxy)), fmaf(Uz, lo(Bxy), -Ux * Bz));
+                const float k2z = fmaf(Ux, hi(Bxy), -Uy * lo(Bxy));
                 Uxy = fma2(bc(A.h_half), k2xy, Txyh); Uz = fmaf(A.h_half, k2z, Tzh);
                 Ux = lo(Uxy); Uy = hi(Uxy);
-                const f2 k3xy = pk(a * fmaf(Uy, Bz, -Uz * hi(Bxy)), a * fmaf(Uz, lo(Bxy), -Ux * Bz));
-                const float k3z = a * fmaf(Ux, hi(Bxy), -Uy * lo(Bxy));
+                const f2 k3xy = pk(fmaf(Uy, Bz, -Uz * hi(Bxy)), fmaf(Uz, lo(Bxy), -Ux * Bz));
+                const float k3z = fmaf(Ux, hi(Bxy), -Uy * lo(Bxy));
                 Uxy = fma2(bc(h), k3xy, Txyh); Uz = fmaf(h, k3z, Tzh);
-                field_at_p(A.fd, fma2(bc(A.h2_2), k3xy, fma2(bc(h), Txyh, xyh)), fmaf(A.h2_2, k3z, fmaf(h, Tzh, zh)), Bxy, Bz);
+                field_at_p(A.fd, a, fma2(bc(A.h2_2), k3xy, fma2(bc(h), Txyh, xyh)), fmaf(A.h2_2, k3z, fmaf(h, Tzh, zh)), Bxy, Bz);
                 Bxy_c = Bxy; Bz_c = Bz;
                 Ux = lo(Uxy); Uy = hi(Uxy);
-                const f2 k4xy = pk(a * fmaf(Uy, Bz, -Uz * hi(Bxy)), a * fmaf(Uz, lo(Bxy), -Ux * Bz));
-                const float k4z = a * fmaf(Ux, hi(Bxy), -Uy * lo(Bxy));
+                const f2 k4xy = pk(fmaf(Uy, Bz, -Uz * hi(Bxy)), fmaf(Uz, lo(Bxy), -Ux * Bz));
+                const float k4z = fmaf(Ux, hi(Bxy), -Uy * lo(Bxy));
                 const f2 dxy = fma2(bc(A.h2_6), add2(add2(k1xy, k2xy), k3xy), mul2(h, Txyh));
                 const float dz = fmaf(A.h2_6, (k1z + k2z) + k3z, h * Tzh);
                 const f2 dTxy = mul2(A.h_6, fma2(bc(2.0f), add2(k2xy, k3xy), add2(k1xy, k4xy)));
