@@ -412,3 +412,33 @@ def test_theta_sharded_scan_equals_the_unsharded_scan(setup, world):
     one = sc.scan_sharded(sc.upload(off, w, d), grids, P, 0, 1, off, collective=True)
     for k in ("best_seed", "best_n_match", "best_chi2", "labels"):
         assert np.array_equal(one[k], whole[k]), k
+
+
+def test_field_reuse_decision_boundary_positions(setup):
+    """Tabulated field: the kernel carries B at a step's start vertex over from the previous step's 4th-stage point only
+    where the two provably differ by less than half an ulp32 of B_max (reading C22; about 25 MeV/c for this
+    table at 2 mm steps).  Seeds from 12 to 60 MeV/c -- both sides of that decision -- end within 1e-3 mm of the oracle,
+    which evaluates B at every vertex, with identical step counts."""
+    cfg, geom, _, events, grids, sc = setup
+    field = synth.make_table_field()
+    cfg3 = synth.CONFIGS[3]
+    ev = synth.generate_events(cfg3, geom, field, 1)[0]
+    u = ev.seed[2:5] / np.linalg.norm(ev.seed[2:5])
+    # |p| of the nodes: the three momentum axes scale the truth direction by 0.12 .. 0.57 independently
+    lo = np.concatenate([ev.seed[:2], 0.12 * 104.97 * u]); step = np.concatenate([[0.0, 0.0], 0.09 * 104.97 * u])
+    g = synth.Grid(lo=lo, step=step, n=np.array([1, 1, 6, 6, 6], dtype=np.int32))
+    p = np.array([np.linalg.norm(g.node(g.unravel(i))[2:5]) for i in range(g.n_seeds)])
+    assert p.min() < 20.0 and p.max() > 50.0 and ((p > 20) & (p < 30)).any()
+    sc3 = api.SeedScanner(geom, field)
+    E3 = sc3.upload(*synth.pack_hits([ev]))
+    P = B.scan_params(cfg3.h_mm, 900, cfg3.window_mm)
+    gpu = sc3.scan(E3, [g], P, per_seed=True, debug=True, best=False)
+    orc = oracle.scan_parallel(geom, field, dict(h=cfg3.h_mm, max_steps=900, window=cfg3.window_mm), ev.wire_id, ev.drift_mm, g)
+    same = gpu["debug"]["n_steps"] == orc["n_steps"]
+    assert (~same).sum() <= 2
+    pos = np.stack([gpu["debug"][k] for k in "xyz"], axis=1)
+    err = np.linalg.norm(pos - orc["final_r"], axis=1)
+    print(f"|p| {p.min():.1f} .. {p.max():.1f} MeV/c, steps {orc['n_steps'].min()} .. {orc['n_steps'].max()}, max position error "
+          f"{err[same].max():.2e} mm (below 25 MeV/c: {err[same & (p < 25)].max():.2e}, above: {err[same & (p >= 25)].max():.2e})")
+    assert err[same].max() < U.POS_TOL_MM
+    sc3.close()
