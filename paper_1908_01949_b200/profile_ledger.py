@@ -7,7 +7,7 @@ needs -lineinfo at compile time), instruction by instruction, and prints
   * executed warp instructions per source line of the kernel file (inlined code is charged to the line of the kernel
     that called it), with the average number of active lanes,
   * the same per named region (line ranges given on the command line),
-  * the opcode histogram.
+  * the opcode histogram, and the fp32 flops the executed instructions carry (thread level, packed forms included).
 Divide by the number of loop iterations (the count of a line that executes once per iteration) to get instructions per
 warp-step.  Used for profiles/r2_scan_ledger_*.md.
 
@@ -23,6 +23,10 @@ import re
 import subprocess
 import sys
 import tempfile
+
+
+# fp32 flops per THREAD instruction (ncu's sass_thread_inst_executed_op_f* metrics do not count the packed forms)
+FP32_FLOPS = {"FFMA": 2, "FMUL": 1, "FADD": 1, "FFMA2": 4, "FMUL2": 2, "FADD2": 2}
 
 
 def disassemble(obj, kernel):
@@ -71,6 +75,7 @@ def main(argv):
     assert len(data) == len(insts), f"{len(insts)} SASS instructions in the object, {len(data)} in the report: not the same build"
     by_line, thr_line, by_op = collections.Counter(), collections.Counter(), collections.Counter()
     total = 0
+    flops = 0
     listing = open(argv[argv.index("--listing") + 1], "w") if "--listing" in argv else None
     listed = 0
     for k, ((text, chain), r) in enumerate(zip(insts, data)):
@@ -88,12 +93,15 @@ def main(argv):
         by_line[outer] += cnt; thr_line[outer] += thr
         op = text.split()[1] if text.startswith("@") else text.split()[0]
         by_op[op.split(".")[0]] += cnt
+        flops += thr * FP32_FLOPS.get(op.split(".")[0], 0)
     if listing:
         listing.write(f"# listed instructions: {listed / per:.1f} of {total / per:.1f} executed warp instructions per unit\n")
         listing.close()
     unit = (lambda c: f"{c / per:8.2f}") if per else (lambda c: f"{c:14d}")
     print(f"kernel {kernel}: {len(insts)} SASS instructions, {total} executed warp instructions" +
           (f", {total / per:.1f} per unit ({per:.0f} units)" if per else ""))
+    print(f"fp32 flops executed (thread level; FFMA 2, FMUL / FADD 1, FFMA2 4, FMUL2 / FADD2 2): {flops}" +
+          (f", {flops / per:.1f} per unit" if per else ""))
     if regions:
         print("\nper region" + (" (instructions per unit)" if per else ""))
         for name, lo, hi in regions:
