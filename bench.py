@@ -45,9 +45,9 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3", choices=["cfg0", "cfg1", "cfg2", "cfg3"])
     ap.add_argument("--events", type=int, default=0, help="events per GPU (0 = the config's own: 256 for cfg3, else 1)")
-    ap.add_argument("--kernel-variant", type=int, default=0, choices=[0, 1, 2],
+    ap.add_argument("--kernel-variant", type=int, default=0, choices=[0, 1, 2, 3],
                     help="0 = production scan kernel, 1 = the two-seeds-per-thread comparison variant, 2 = the lane-refill "
-                         "comparison variant")
+                         "comparison variant, 3 = the production kernel with the field reuse off (A / B)")
     ap.add_argument("--no-secondary", action="store_true", help="skip the short configs[1] measurement")
     ap.add_argument("--shard", default="auto", choices=["auto", "events", "theta"],
                     help="with N GPUs: 'events' = every rank scans its own events (weak scaling, no collective); 'theta' = "

@@ -91,7 +91,11 @@ typedef struct {
  *   the long track of the next, and a per-step warp vote ends the warp: every lane stays live (32.0 of 32 in the step
  *   against 29.3 / 30.8) but the second seeds are out of step with their z0 neighbours and the lookup and live-wire
  *   code pay more than the step saves: measured slower (profiles/r2_refill_kernel.md), kept as the comparison point;
- *   per-seed n_match, chi2, positions, best seed and labels are bit-identical, tests/test_gpu_refill.py checks it. */
+ *   per-seed n_match, chi2, positions, best seed and labels are bit-identical, tests/test_gpu_refill.py checks it;
+ *   3 = the production kernel with the field reuse off (tabulated field: B is evaluated at every step's start vertex
+ *   instead of being carried over from the previous step's 4th-stage point where that is provably below fp32
+ *   resolution, reading C22): the A / B switch for that one decision (tests/test_gpu_edges.py,
+ *   `bench.py --kernel-variant 3`); identical to 0 in the uniform field. */
 typedef struct {
     double h_mm;
     int32_t max_steps;

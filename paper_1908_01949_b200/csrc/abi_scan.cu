@@ -49,7 +49,7 @@ int32_t check_params(const cdc_scan_params *p, const char *who)
     if (!(p->window_mm > 0.0)) CDC_FAIL(CDC_ERR_INVALID, std::string(who) + ": window <= 0");
     if (!(p->eloss_MeV_per_mm >= 0.0)) CDC_FAIL(CDC_ERR_INVALID, std::string(who) + ": negative energy loss");
     if (p->charge != 1 && p->charge != -1) CDC_FAIL(CDC_ERR_INVALID, std::string(who) + ": charge must be +-1");
-    if (p->kernel_variant < 0 || p->kernel_variant > 2) CDC_FAIL(CDC_ERR_INVALID, std::string(who) + ": kernel_variant must be 0, 1 or 2");
+    if (p->kernel_variant < 0 || p->kernel_variant > 3) CDC_FAIL(CDC_ERR_INVALID, std::string(who) + ": kernel_variant must be 0, 1, 2 or 3");
     return CDC_OK;
 }
 

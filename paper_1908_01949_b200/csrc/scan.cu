@@ -336,6 +336,7 @@ cudaError_t launch_seed_scan(const ScanLaunch &L, cudaStream_t s, cudaEvent_t k0
     // the next power of two >= that)
     A.reuse_c = (float)(h * h * h / 6.0 * (double)L.fd.grad_max); A.reuse_b2 = L.b_max * L.b_max;
     A.reuse_eps = (float)(ldexp(1.0, -24) * (double)L.b_max);
+    if (L.variant == 3) A.reuse_eps = -1.0f;          // params.kernel_variant = 3: this kernel with the field reuse off (A / B)
     A.max_steps = L.max_steps; A.margin = L.margin;
     A.n_match = L.d_n_match; A.chi2 = L.d_chi2; A.debug = L.d_debug;
     A.best_key = (unsigned long long *)L.d_best_key;

@@ -442,3 +442,25 @@ def test_field_reuse_decision_boundary_positions(setup):
           f"{err[same].max():.2e} mm (below 25 MeV/c: {err[same & (p < 25)].max():.2e}, above: {err[same & (p >= 25)].max():.2e})")
     assert err[same].max() < U.POS_TOL_MM
     sc3.close()
+
+
+def test_field_reuse_on_and_off_give_the_same_tracks(setup):
+    """A / B of the one decision of reading C22 (params.kernel_variant = 3 evaluates B at every start vertex): per seed the
+    same step counts, final positions within 2e-5 mm of one another (both within 1e-3 mm of the oracle, test above and
+    test_gpu_parity.py), n_match equal up to a handful of window-edge cases, and the same exact best seed, chi2 and labels."""
+    cfg3, geom, field, events, grids = U.make_workload(3, n_events=3, grid_n=9)
+    sc3 = api.SeedScanner(geom, field)
+    out = []
+    for variant in (0, 3):
+        E3 = sc3.upload(*synth.pack_hits(events))
+        out.append(sc3.scan(E3, grids, U.gpu_params(cfg3, kernel_variant=variant), per_seed=True, debug=True))
+    a, b = out
+    assert np.array_equal(a["debug"]["n_steps"], b["debug"]["n_steps"])
+    d = np.sqrt(sum((a["debug"][k] - b["debug"][k]) ** 2 for k in "xyz"))
+    n_diff = int((a["n_match"] != b["n_match"]).sum())
+    print(f"reuse on / off: {a['n_match'].size} seeds, max position difference {d.max():.2e} mm, n_match differs on {n_diff}")
+    assert d.max() < 2e-5
+    assert n_diff <= max(2, int(2e-4 * a["n_match"].size))
+    for k in ("best_seed", "best_n_match", "best_chi2", "labels"):
+        assert np.array_equal(a[k], b[k]), k
+    sc3.close()
