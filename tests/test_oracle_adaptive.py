@@ -120,3 +120,54 @@ def test_adaptive_scan_finds_the_same_hits(geom, table_field):
         assert ad["n_steps"] < 0.6 * fx["n_steps"] and abs(ad["units"] - fx["n_steps"]) <= 2
         assert abs(ad["n_match"] - fx["n_match"]) <= 1 and abs(ad["chi2"] - fx["chi2"]) < 0.1
         assert np.linalg.norm(ad["r"] - fx["r"]) < 2.0 * cfg.h_mm + 1e-3      # ends within one long step of it
+
+
+def test_diagnostic_margins_against_independent_values(geom, uniform_field, table_field):
+    """The decision and boundary margins the adaptive evaluation returns are what the parity protocol's exception classes
+    rest on (tests/parity_util.compare_scan_adaptive), so they are pinned against values formed without them:
+    (i) uniform field, tol -> 0 (every trial at level 0; the estimate at a vertex is h^2 times the maximum component of the
+        closed form -(c^3 h^2 / 4) J T + (c^4 h^3 / 4) T of the test above): margin_tol = min |est - tol| / tol, margin_up =
+        min |est - tol/32| / (tol/32), and the same two distances over h^2;
+    (ii) tabulated field: the track is re-traced here vertex by vertex with the one-step routine (pinned elsewhere) and
+        r0_margin = min_n>=1 | rho_n - R0 |, exit_margin = min_n>=1 min(| |z_n| - z_half |, | rho_n - r_out |)."""
+    cfg = synth.CONFIGS[1]
+    b = _bound(geom, uniform_field, cfg, max_steps=400)
+    pt, p = 90.0, 104.97
+    seed = np.array([0.4, -100.0, pt * math.cos(1.0), pt * math.sin(1.0), math.sqrt(p * p - pt * pt)])
+    h, tol = cfg.h_mm, 1e-13
+    w = np.array([5], dtype=np.int32); d = np.array([1.0], dtype=np.float32)
+    r = oracle.eval_seed_adaptive(b, w, d, seed, tol, 16.0)
+    assert r["n_level"][0] == r["n_steps"] > 100
+    # the estimate at every vertex from the closed form (maximum norm, as the controller takes it), T_n from the one-step routine
+    c = -KAPPA / p                                   # a B_z, electron
+    pos = np.array([geom.R0_mm * math.cos(seed[0]), geom.R0_mm * math.sin(seed[0]), seed[1]]); T = seed[2:5] / p
+    est = []
+    for n in range(r["n_steps"]):
+        vx = -(c ** 3 * h ** 2 / 4.0) * T[1] + (c ** 4 * h ** 3 / 4.0) * T[0]
+        vy = (c ** 3 * h ** 2 / 4.0) * T[0] + (c ** 4 * h ** 3 / 4.0) * T[1]
+        est.append(h ** 2 * max(abs(vx), abs(vy)))
+        pos, T = oracle.rkn_step(b, c, h, pos, T)
+    est = np.array(est)
+    assert r["margin_tol"] == pytest.approx(np.min(np.abs(est - tol)) / tol, rel=1e-5)
+    assert r["margin_up"] == pytest.approx(np.min(np.abs(est - tol / 32)) / (tol / 32), rel=1e-5)
+    assert r["kmargin_tol"] == pytest.approx(np.min(np.abs(est - tol)) / h ** 2, rel=1e-5)
+    assert r["kmargin_up"] == pytest.approx(np.min(np.abs(est - tol / 32)) / h ** 2, rel=1e-5)
+    # (ii)
+    cfg3 = synth.CONFIGS[3]
+    ev = synth.generate_events(cfg3, geom, table_field, 1)[0]
+    b3 = _bound(geom, table_field, cfg3)
+    r3 = oracle.eval_seed_adaptive(b3, ev.wire_id, ev.drift_mm, ev.seed, 1e-13, 16.0)
+    th, z0, px, py, pz = ev.seed
+    p0 = math.sqrt(px * px + py * py + pz * pz)
+    pos = np.array([geom.R0_mm * math.cos(th), geom.R0_mm * math.sin(th), z0]); T = np.array([px, py, pz]) / p0
+    a = -KAPPA / p0
+    r0m = exm = float("inf")
+    for n in range(r3["n_steps"]):
+        pos, T = oracle.rkn_step(b3, a, cfg3.h_mm, pos, T)
+        rho = math.sqrt(pos[0] * pos[0] + pos[1] * pos[1])
+        r0m = min(r0m, abs(rho - geom.R0_mm))
+        exm = min(exm, abs(abs(pos[2]) - geom.z_half_mm), abs(rho - geom.r_out_mm))
+    assert np.array_equal(pos, r3["r"])                                  # the same track
+    assert r3["r0_margin"] == pytest.approx(r0m, rel=1e-12, abs=1e-12)
+    assert r3["exit_margin"] == pytest.approx(exm, rel=1e-12, abs=1e-12)
+    assert 0.0 < r3["exit_margin"] < cfg3.h_mm and r3["r0_margin"] < cfg3.h_mm     # a vertex near the exit / near R0 exists
