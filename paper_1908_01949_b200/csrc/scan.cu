@@ -225,9 +225,12 @@ __global__ void __launch_bounds__(kBlock, FIELD == 0 ? SCAN_MB0 : SCAN_MB1) seed
             const float dTz = A.h_6 * fmaf(2.0f, k2z + k3z, k1z + k4z);
             sdxy = fma2(bc(h), Txyl, dxy); sdz = fmaf(h, Tzl, dz);
             comp_add2(xyh, xyl, sdxy);
-            comp_add(zh, zl, sdz);
             comp_add2(Txyh, Txyl, fma2(dTxy, bc(epsT), dTxy));
-            comp_add(Tzh, Tzl, fmaf(dTz, epsT, dTz));
+            {   // z and T_z take the same compensated update: one packed pair for the two (same operations, same rounding)
+                f2 zT_h = pk(zh, Tzh), zT_l = pk(zl, Tzl);
+                comp_add2(zT_h, zT_l, pk(sdz, fmaf(dTz, epsT, dTz)));
+                zh = lo(zT_h); Tzh = hi(zT_h); zl = lo(zT_l); Tzl = hi(zT_l);
+            }
         }
 
         // ---- A6: live wires over interval n (scored only if the interval starts in the gas)
